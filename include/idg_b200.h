@@ -1,0 +1,149 @@
+/*
+ * idg_b200.h -- C ABI of the B200-native Image Domain Gridding hot path.
+ *
+ * Method: van der Tol, Veenboer & Offringa, "Image Domain Gridding: a fast method for
+ * convolutional resampling of visibilities", arXiv 1909.07226.  Citations are lines of
+ * /root/reference/PAPER.md plus the section / equation / algorithm they fall in; "R<n>"
+ * names a reading of a garbled or silent passage listed in DESIGN.md.
+ *
+ * Conventions shared by every entry point
+ *   - Every function returns int: IDG_OK (0) or a negative idg_status.  No exceptions, no
+ *     aborts, nothing printed.  idg_strerror() names a code; idg_last_cuda_error() returns the
+ *     cudaError_t behind the last IDG_ERR_CUDA of the calling thread.
+ *   - "_dev" pointers are CUDA device pointers owned by the caller; "_host" pointers are host
+ *     memory owned by the caller.  The library never frees or keeps caller memory beyond the
+ *     call (asynchronous work on `cuda_stream` excepted: buffers must stay valid until the
+ *     stream has run it).  `cuda_stream` is a cudaStream_t passed as void* (NULL = default).
+ *   - idg_grid / idg_degrid and the stage entry points are asynchronous on `cuda_stream` and
+ *     never synchronise it; idg_plan_create and the *_host entry points synchronise.
+ *   - Layouts (C order, complex64 = two float32, re then im):
+ *       uvw      [B][T][3]                 float32 metres (u, v, w)
+ *       vis      [B][T][C][4]              complex64, polarisations XX, XY, YX, YY (row-major 2x2)
+ *       aterms   [slots][stations][N][N][4] complex64 Jones matrices, pixel [y][x], row-major 2x2
+ *       taper    [N][N]                    float32, pixel [y][x]
+ *       subgrids [P][4][N][N]              complex64, [pol][y][x]
+ *       grid     [4][L][L]                 complex64, [pol][y][x]; x <-> u <-> l fastest
+ *   - A "visibility" is one (baseline, timestep, channel) sample with all four polarisations
+ *     (section 5.3).
+ */
+#ifndef IDG_B200_H
+#define IDG_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  IDG_OK = 0,
+  IDG_ERR_INVALID_ARG = -1,
+  IDG_ERR_OUT_OF_MEMORY = -2,
+  IDG_ERR_CUDA = -3,
+  IDG_ERR_PLAN_MISMATCH = -4,
+  IDG_ERR_UNSUPPORTED_SUBGRID_SIZE = -5
+} idg_status;
+
+#define IDG_PLAN_FORCE_BLOCKS 1 /* flags: blocks end only on max_timesteps / A-term slot (sweep mode) */
+
+/* Partitioning parameters (section 3.2; readings R10-R12).  All explicit. */
+typedef struct {
+  int32_t grid_size;      /* L, even, >= subgrid_size */
+  int32_t subgrid_size;   /* N in {16, 24, 32, 48} */
+  int32_t kernel_size;    /* pixels reserved for taper / w / A-term support, 0 < kernel_size < N */
+  int32_t max_timesteps;  /* per subgrid, >= 1 */
+  int32_t max_channels;   /* per subgrid, power of two */
+  int32_t aterm_interval; /* timesteps per A-term slot, >= 1 (R5: a block never spans two slots) */
+  int32_t flags;          /* IDG_PLAN_FORCE_BLOCKS or 0 */
+  int32_t reserved;       /* must be 0 */
+  double image_size;      /* S: direction-cosine extent of the image; grid cell = 1/S wavelengths */
+  double w_step;          /* w-layer thickness in wavelengths; 0 -> w0 = 0 for every subgrid (R4) */
+} idg_plan_params;
+
+/* One subgrid of the partition: 48 bytes, the bit-exact contract (Alg. 1
+ * PAPER.md:276; D6 of SURVEY.md).  Centre pixel of the subgrid on the grid = (x0 + N/2, y0 + N/2);
+ * u0 = (x0 + N/2 - L/2)/S (R3); w0 = (w_index + 0.5) w_step (R4). */
+typedef struct {
+  int32_t baseline, station1, station2, time_begin, n_time, chan_begin, n_chan, aterm_slot, x0, y0,
+      w_index, reserved;
+} idg_subgrid_meta;
+
+typedef struct idg_plan idg_plan; /* opaque; owns metadata (host + device), adder work lists,
+                                     the [P][4][N][N] subgrid scratch buffer and staging buffers */
+
+const char *idg_strerror(int code);
+int idg_last_cuda_error(void);
+
+/* ---- planner (a0): section 3.2, Fig. 2; readings R10-R12 -----
+ * Partitions every baseline's (time x channel) samples into blocks whose uv extent in grid
+ * pixels plus kernel_size fits N, with one A-term slot and one w layer per block.  Runs on the
+ * GPU (one walk per baseline, count -> scan -> emit), double arithmetic without FMA contraction;
+ * the metadata is bit-identical to the step-by-step rule in DESIGN.md.  Synchronises the stream.
+ *   uvw_dev        [B][T][3] float32 metres, device
+ *   freqs_host     [C] float64 Hz, host (copied)
+ *   baselines_host [B][2] int32 station pairs, host (copied)
+ * Samples whose subgrid would leave the grid are skipped and counted, not an error.
+ * Errors: IDG_ERR_INVALID_ARG (null pointers, bad params), IDG_ERR_UNSUPPORTED_SUBGRID_SIZE,
+ * IDG_ERR_OUT_OF_MEMORY, IDG_ERR_CUDA.  *out is NULL on error. */
+int idg_plan_create(idg_plan **out, const idg_plan_params *prm, const float *uvw_dev,
+                    const double *freqs_host, const int32_t *baselines_host, int32_t B, int32_t T,
+                    int32_t C, int32_t n_stations, void *cuda_stream);
+/* Builds a plan from caller-supplied metadata (host, P entries; validated against the grid and
+ * the array shapes) instead of running the planner: for tests and for externally made plans. */
+int idg_plan_from_metadata(idg_plan **out, const idg_plan_params *prm,
+                           const idg_subgrid_meta *meta_host, int64_t P, const double *freqs_host,
+                           int32_t B, int32_t T, int32_t C, int32_t n_stations, void *cuda_stream);
+int idg_plan_size(const idg_plan *plan, int64_t *n_subgrids, int64_t *n_planned_vis,
+                  int64_t *n_skipped_vis);
+/* Copies min(P, capacity) entries to out_host; IDG_ERR_INVALID_ARG if capacity < P. */
+int idg_plan_metadata(const idg_plan *plan, idg_subgrid_meta *out_host, int64_t capacity);
+/* Device pointer of the plan-owned [P][4][N][N] complex64 scratch (valid until destroy). */
+int idg_plan_subgrids(const idg_plan *plan, void **subgrids_dev);
+void idg_plan_destroy(idg_plan *plan);
+
+/* ---- Algorithm 1 without its last line: gridder -> subgrid FFT -> adder.
+ * ACCUMULATES into grid_dev (Alg. 1 zeroes V once; zeroing is the caller's). */
+int idg_grid(const idg_plan *plan, const float *uvw_dev, const void *vis_dev,
+             const void *aterms_dev, const float *taper_dev, void *grid_dev, void *cuda_stream);
+/* ---- Algorithm 2 after its first two lines: splitter -> subgrid IFFT ->
+ * degridder.  Overwrites every planned visibility; skipped ones are set to 0. */
+int idg_degrid(const idg_plan *plan, const float *uvw_dev, const void *grid_dev,
+               const void *aterms_dev, const float *taper_dev, void *vis_out_dev,
+               void *cuda_stream);
+
+/* ---- the same two calls on HOST buffers (pinned or pageable): copy in, run, copy out,
+ * synchronise.  Device staging buffers are owned by the plan (allocated on first use).
+ * idg_grid_host adds into grid_host (which is read, accumulated into on the device, and
+ * written back). */
+int idg_grid_host(idg_plan *plan, const float *uvw_host, const void *vis_host,
+                  const void *aterms_host, int32_t n_slots, const float *taper_host,
+                  void *grid_host, void *cuda_stream);
+int idg_degrid_host(idg_plan *plan, const float *uvw_host, const void *grid_host,
+                    const void *aterms_host, int32_t n_slots, const float *taper_host,
+                    void *vis_out_host, void *cuda_stream);
+
+/* ---- stage-level entry points (parity tests, per-stage timing); same conventions ------------
+ * a1 gridder: Eq. 25, Alg. 1, section 3.4 PAPER.md:247-249:
+ *   Sg[y][x] = taper A1^H (sum_k Y_k exp(+2 pi i (du l_x + dv m_y + dw n'_xy))) A2  -> subgrids */
+int idg_gridder(const idg_plan *plan, const float *uvw_dev, const void *vis_dev,
+                const void *aterms_dev, const float *taper_dev, void *subgrids_dev,
+                void *cuda_stream);
+/* a2 / a5 subgrid FFT: centred 2-D DFT of every plane in place, scale 1/N^2 both ways (R6);
+ * direction -1 = forward exp(-..), +1 = inverse. */
+int idg_subgrid_fft(const idg_plan *plan, void *subgrids_dev, int32_t direction,
+                    void *cuda_stream);
+/* a3 adder: grid[pol][y0+b][x0+a] += V_p[pol][b][a] (Eq. 24). */
+int idg_adder(const idg_plan *plan, const void *subgrids_dev, void *grid_dev, void *cuda_stream);
+/* a4 splitter: V_p[pol][b][a] = grid[pol][y0+b][x0+a]. */
+int idg_splitter(const idg_plan *plan, const void *grid_dev, void *subgrids_dev,
+                 void *cuda_stream);
+/* a6 degridder: Alg. 2: Dg = A1 (taper Ip) A2^H per pixel, then
+ *   Y_k = sum_xy Dg[y][x] exp(-2 pi i (du l_x + dv m_y + dw n'_xy)) -> vis_out (planned only). */
+int idg_degridder(const idg_plan *plan, const float *uvw_dev, const void *subgrids_dev,
+                  const void *aterms_dev, const float *taper_dev, void *vis_out_dev,
+                  void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IDG_B200_H */
