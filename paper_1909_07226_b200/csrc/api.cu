@@ -1,0 +1,201 @@
+// api.cu -- the C ABI of include/idg_b200.h: argument checks, plan ownership, stage sequencing.
+#include <algorithm>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+namespace idg {
+
+static thread_local int g_last_cuda_error = 0;
+void set_last_cuda_error(cudaError_t e) { g_last_cuda_error = (int)e; }
+
+static bool supported_size(int n) { return n == 16 || n == 24 || n == 32 || n == 48; }
+static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+static int check_params(const idg_plan_params *p) {
+  if (!p) return IDG_ERR_INVALID_ARG;
+  if (!supported_size(p->subgrid_size)) return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
+  if (p->grid_size < p->subgrid_size || (p->grid_size & 1)) return IDG_ERR_INVALID_ARG;
+  if (p->kernel_size <= 0 || p->kernel_size >= p->subgrid_size) return IDG_ERR_INVALID_ARG;
+  if (p->max_timesteps < 1 || p->aterm_interval < 1) return IDG_ERR_INVALID_ARG;
+  if (!is_pow2(p->max_channels) || p->max_channels > 256) return IDG_ERR_INVALID_ARG;
+  if (p->reserved != 0 || (p->flags & ~IDG_PLAN_FORCE_BLOCKS)) return IDG_ERR_INVALID_ARG;
+  if (!(p->image_size > 0.0) || !(p->image_size < 1.4) || !(p->w_step >= 0.0)) return IDG_ERR_INVALID_ARG;
+  return IDG_OK;
+}
+
+// Bucket the subgrids by the grid tiles they overlap (stable counting sort in p) and cut every
+// tile's list into work items of at most kAdderChunk subgrids.
+static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
+  const int N = pl->prm.subgrid_size, L = pl->prm.grid_size, TS = kAdderTile;
+  const int nt = (L + TS - 1) / TS;
+  std::vector<int64_t> offs((size_t)nt * nt + 1, 0);
+  for (const auto &m : pl->meta_host)
+    for (int ty = m.y0 / TS; ty <= (m.y0 + N - 1) / TS; ++ty)
+      for (int tx = m.x0 / TS; tx <= (m.x0 + N - 1) / TS; ++tx) ++offs[(size_t)ty * nt + tx + 1];
+  for (size_t i = 1; i < offs.size(); ++i) offs[i] += offs[i - 1];
+  const int64_t total = offs.back();
+  std::vector<int32_t> list((size_t)total);
+  std::vector<int64_t> cur(offs.begin(), offs.end() - 1);
+  for (int64_t p = 0; p < pl->P; ++p) {
+    const auto &m = pl->meta_host[(size_t)p];
+    for (int ty = m.y0 / TS; ty <= (m.y0 + N - 1) / TS; ++ty)
+      for (int tx = m.x0 / TS; tx <= (m.x0 + N - 1) / TS; ++tx)
+        list[(size_t)cur[(size_t)ty * nt + tx]++] = (int32_t)p;
+  }
+  std::vector<AdderItem> items;
+  for (int ty = 0; ty < nt; ++ty)
+    for (int tx = 0; tx < nt; ++tx) {
+      const int64_t b = offs[(size_t)ty * nt + tx], e = offs[(size_t)ty * nt + tx + 1];
+      for (int64_t s = b; s < e; s += kAdderChunk)
+        items.push_back(AdderItem{tx * TS, ty * TS, (int32_t)s, (int32_t)std::min<int64_t>(e, s + kAdderChunk)});
+    }
+  pl->n_adder_items = (int64_t)items.size();
+  if (total > 0) {
+    IDG_CUDA_TRY(cudaMalloc(&pl->adder_list_dev, sizeof(int32_t) * (size_t)total));
+    IDG_CUDA_TRY(cudaMalloc(&pl->adder_items_dev, sizeof(AdderItem) * items.size()));
+    IDG_CUDA_TRY(cudaMemcpyAsync(pl->adder_list_dev, list.data(), sizeof(int32_t) * (size_t)total,
+                                 cudaMemcpyHostToDevice, stream));
+    IDG_CUDA_TRY(cudaMemcpyAsync(pl->adder_items_dev, items.data(), sizeof(AdderItem) * items.size(),
+                                 cudaMemcpyHostToDevice, stream));
+    IDG_CUDA_TRY(cudaStreamSynchronize(stream));  // the host vectors go out of scope
+  }
+  return IDG_OK;
+}
+
+// Everything a plan owns besides the metadata: frequencies, scratch, adder lists.
+static int finish_plan(idg_plan *pl, const double *freqs_host, cudaStream_t stream) {
+  const int N = pl->prm.subgrid_size;
+  pl->P = (int64_t)pl->meta_host.size();
+  pl->max_n_time = 0; pl->max_n_chan = 0;
+  for (const auto &m : pl->meta_host) {
+    pl->max_n_time = std::max(pl->max_n_time, m.n_time);
+    pl->max_n_chan = std::max(pl->max_n_chan, m.n_chan);
+  }
+  IDG_CUDA_TRY(cudaMalloc(&pl->freqs_dev, sizeof(double) * pl->C));
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->freqs_dev, freqs_host, sizeof(double) * pl->C,
+                               cudaMemcpyHostToDevice, stream));
+  IDG_CUDA_TRY(cudaStreamSynchronize(stream));
+  if (pl->P > 0)
+    IDG_CUDA_TRY(cudaMalloc(&pl->subgrids_dev, sizeof(float2) * 4 * N * N * (size_t)pl->P));
+  return build_adder_lists(pl, stream);
+}
+
+}  // namespace idg
+
+using namespace idg;
+
+extern "C" {
+
+const char *idg_strerror(int code) {
+  switch (code) {
+    case IDG_OK: return "ok";
+    case IDG_ERR_INVALID_ARG: return "invalid argument";
+    case IDG_ERR_OUT_OF_MEMORY: return "out of memory";
+    case IDG_ERR_CUDA: return "CUDA error (see idg_last_cuda_error)";
+    case IDG_ERR_PLAN_MISMATCH: return "metadata does not match the plan parameters or array shapes";
+    case IDG_ERR_UNSUPPORTED_SUBGRID_SIZE: return "subgrid size must be 16, 24, 32 or 48";
+    default: return "unknown error code";
+  }
+}
+
+int idg_last_cuda_error(void) { return g_last_cuda_error; }
+
+void idg_plan_destroy(idg_plan *pl) {
+  if (!pl) return;
+  cudaFree(pl->meta_dev); cudaFree(pl->freqs_dev); cudaFree(pl->subgrids_dev);
+  cudaFree(pl->adder_list_dev); cudaFree(pl->adder_items_dev);
+  cudaFree(pl->h_uvw_dev); cudaFree(pl->h_vis_dev); cudaFree(pl->h_aterms_dev);
+  cudaFree(pl->h_grid_dev); cudaFree(pl->h_taper_dev);
+  delete pl;
+}
+
+int idg_plan_create(idg_plan **out, const idg_plan_params *prm, const float *uvw_dev,
+                    const double *freqs_host, const int32_t *baselines_host, int32_t B, int32_t T,
+                    int32_t C, int32_t n_stations, void *cuda_stream) {
+  if (out) *out = nullptr;
+  if (!out || !uvw_dev || !freqs_host || !baselines_host || B < 1 || T < 1 || C < 1 || n_stations < 1)
+    return IDG_ERR_INVALID_ARG;
+  int rc = check_params(prm);
+  if (rc != IDG_OK) return rc;
+  for (int32_t b = 0; b < B; ++b)
+    if (baselines_host[2 * b] < 0 || baselines_host[2 * b] >= n_stations ||
+        baselines_host[2 * b + 1] < 0 || baselines_host[2 * b + 1] >= n_stations)
+      return IDG_ERR_INVALID_ARG;
+  idg_plan *pl = new (std::nothrow) idg_plan();
+  if (!pl) return IDG_ERR_OUT_OF_MEMORY;
+  pl->prm = *prm; pl->B = B; pl->T = T; pl->C = C; pl->n_stations = n_stations;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  rc = run_planner(*prm, uvw_dev, freqs_host, baselines_host, B, T, C, pl->meta_host, &pl->meta_dev,
+                   &pl->n_planned, &pl->n_skipped, stream);
+  if (rc == IDG_OK) rc = finish_plan(pl, freqs_host, stream);
+  if (rc != IDG_OK) { idg_plan_destroy(pl); return rc; }
+  *out = pl;
+  return IDG_OK;
+}
+
+int idg_plan_from_metadata(idg_plan **out, const idg_plan_params *prm,
+                           const idg_subgrid_meta *meta_host, int64_t P, const double *freqs_host,
+                           int32_t B, int32_t T, int32_t C, int32_t n_stations, void *cuda_stream) {
+  if (out) *out = nullptr;
+  if (!out || (!meta_host && P > 0) || P < 0 || !freqs_host || B < 1 || T < 1 || C < 1 || n_stations < 1)
+    return IDG_ERR_INVALID_ARG;
+  int rc = check_params(prm);
+  if (rc != IDG_OK) return rc;
+  const int N = prm->subgrid_size, L = prm->grid_size;
+  int64_t planned = 0;
+  for (int64_t p = 0; p < P; ++p) {
+    const idg_subgrid_meta &m = meta_host[p];
+    const bool ok = m.baseline >= 0 && m.baseline < B && m.station1 >= 0 && m.station1 < n_stations &&
+                    m.station2 >= 0 && m.station2 < n_stations && m.time_begin >= 0 && m.n_time >= 1 &&
+                    m.time_begin + m.n_time <= T && m.chan_begin >= 0 && m.n_chan >= 1 &&
+                    m.n_chan <= 256 && m.chan_begin + m.n_chan <= C && m.aterm_slot >= 0 &&
+                    m.x0 >= 0 && m.y0 >= 0 && m.x0 + N <= L && m.y0 + N <= L;
+    if (!ok) return IDG_ERR_PLAN_MISMATCH;
+    planned += (int64_t)m.n_time * m.n_chan;
+  }
+  idg_plan *pl = new (std::nothrow) idg_plan();
+  if (!pl) return IDG_ERR_OUT_OF_MEMORY;
+  pl->prm = *prm; pl->B = B; pl->T = T; pl->C = C; pl->n_stations = n_stations;
+  pl->meta_host.assign(meta_host, meta_host + P);
+  pl->n_planned = planned;
+  pl->n_skipped = (int64_t)B * T * C - planned;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  rc = IDG_OK;
+  if (P > 0) {
+    cudaError_t e = cudaMalloc(&pl->meta_dev, sizeof(idg_subgrid_meta) * (size_t)P);
+    if (e == cudaSuccess)
+      e = cudaMemcpyAsync(pl->meta_dev, meta_host, sizeof(idg_subgrid_meta) * (size_t)P,
+                          cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) { set_last_cuda_error(e); rc = IDG_ERR_CUDA; }
+  }
+  if (rc == IDG_OK) rc = finish_plan(pl, freqs_host, stream);
+  if (rc != IDG_OK) { idg_plan_destroy(pl); return rc; }
+  *out = pl;
+  return IDG_OK;
+}
+
+int idg_plan_size(const idg_plan *pl, int64_t *n_subgrids, int64_t *n_planned_vis,
+                  int64_t *n_skipped_vis) {
+  if (!pl) return IDG_ERR_INVALID_ARG;
+  if (n_subgrids) *n_subgrids = pl->P;
+  if (n_planned_vis) *n_planned_vis = pl->n_planned;
+  if (n_skipped_vis) *n_skipped_vis = pl->n_skipped;
+  return IDG_OK;
+}
+
+int idg_plan_metadata(const idg_plan *pl, idg_subgrid_meta *out_host, int64_t capacity) {
+  if (!pl || (!out_host && pl->P > 0) || capacity < pl->P) return IDG_ERR_INVALID_ARG;
+  if (pl->P > 0) std::memcpy(out_host, pl->meta_host.data(), sizeof(idg_subgrid_meta) * (size_t)pl->P);
+  return IDG_OK;
+}
+
+int idg_plan_subgrids(const idg_plan *pl, void **subgrids_dev) {
+  if (!pl || !subgrids_dev) return IDG_ERR_INVALID_ARG;
+  *subgrids_dev = pl->subgrids_dev;
+  return IDG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,101 @@
+// common.cuh -- internal declarations of libidg_b200 (CUDA, sm_100a only).
+// Product code: shares nothing with oracle/.  See include/idg_b200.h for the boundary.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/idg_b200.h"
+
+namespace idg {
+
+constexpr double kSpeedOfLight = 299792458.0;
+constexpr int kAdderTile = 32;        // grid tile edge owned by one adder work item
+constexpr int kAdderChunk = 48;       // max subgrids accumulated by one work item
+
+struct AdderItem {                    // one unit of adder work: a grid tile and a slice of its list
+  int32_t tile_x, tile_y;             // tile origin on the grid (pixels)
+  int32_t begin, end;                 // range in adder_list
+};
+
+}  // namespace idg
+
+struct idg_plan {
+  idg_plan_params prm{};
+  int32_t B = 0, T = 0, C = 0, n_stations = 0;
+  int64_t P = 0, n_planned = 0, n_skipped = 0;
+  int32_t max_n_time = 0, max_n_chan = 0;
+  std::vector<idg_subgrid_meta> meta_host;
+  idg_subgrid_meta *meta_dev = nullptr;
+  double *freqs_dev = nullptr;        // [C] Hz
+  float2 *subgrids_dev = nullptr;     // [P][4][N][N]
+  // adder: subgrids bucketed by the grid tiles they overlap (stable in p -> fixed order)
+  int32_t *adder_list_dev = nullptr;  // subgrid indices, grouped by tile
+  idg::AdderItem *adder_items_dev = nullptr;
+  int64_t n_adder_items = 0;
+  // staging for the *_host entry points
+  float *h_uvw_dev = nullptr;
+  float2 *h_vis_dev = nullptr, *h_aterms_dev = nullptr, *h_grid_dev = nullptr;
+  float *h_taper_dev = nullptr;
+  int64_t h_aterm_slots = 0;
+};
+
+namespace idg {
+
+void set_last_cuda_error(cudaError_t e);
+
+#define IDG_CUDA_TRY(expr)                                   \
+  do {                                                       \
+    cudaError_t _e = (expr);                                 \
+    if (_e != cudaSuccess) {                                 \
+      idg::set_last_cuda_error(_e);                          \
+      return _e == cudaErrorMemoryAllocation ? IDG_ERR_OUT_OF_MEMORY : IDG_ERR_CUDA; \
+    }                                                        \
+  } while (0)
+
+// planner (plan.cu)
+int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *freqs_host,
+                const int32_t *baselines_host, int32_t B, int32_t T, int32_t C,
+                std::vector<idg_subgrid_meta> &meta_out, idg_subgrid_meta **meta_dev_out,
+                int64_t *planned, int64_t *skipped, cudaStream_t stream);
+
+// stage launchers (one .cu each); all asynchronous on `stream`
+int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
+                   const float *taper, float2 *subgrids, cudaStream_t stream);
+int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgrids,
+                     const float2 *aterms, const float *taper, float2 *vis_out,
+                     cudaStream_t stream);
+int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream);
+int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cudaStream_t stream);
+int launch_splitter(const idg_plan *plan, const float2 *grid, float2 *subgrids,
+                    cudaStream_t stream);
+
+// packed FP32 FMA (sm_100 FFMA2): d = a * b + c on both halves
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+  unsigned long long ra, rb, rc, rd;
+  ra = *reinterpret_cast<unsigned long long *>(&a);
+  rb = *reinterpret_cast<unsigned long long *>(&b);
+  rc = *reinterpret_cast<unsigned long long *>(&c);
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+  return *reinterpret_cast<float2 *>(&rd);
+}
+
+// acc += v * (c + i s) for a complex accumulator, as two FFMA2
+__device__ __forceinline__ void cmac(float2 &acc, float2 v, float c, float s) {
+  acc = ffma2(make_float2(v.x, v.x), make_float2(c, s), acc);
+  acc = ffma2(make_float2(v.y, v.y), make_float2(-s, c), acc);
+}
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ float2 cmul_conj_a(float2 a, float2 b) {  // conj(a) * b
+  return make_float2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+}
+__device__ __forceinline__ float2 cmul_conj_b(float2 a, float2 b) {  // a * conj(b)
+  return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+
+}  // namespace idg

@@ -1,0 +1,178 @@
+// degridder.cu -- row a6: predict the visibilities of every block from its subgrid image.
+//
+// Alg. 2 inner loops (R9: I[i,j] there is I_p[i,j]), polarised form
+// (PAPER.md:249), exact adjoint of the gridder:
+//   Dg[y][x]   = A1[y][x] (taper[y][x] Ip[y][x]) A2[y][x]^H                      (R5)
+//   Y[b][t][c] = sum_{y,x} Dg[y][x] exp(-2 pi i (du l_x + dv m_y + dw n'_xy))
+//
+// B200 design: one CTA per subgrid.  The reduction axis is the pixels, so here the THREADS own
+// visibilities (one timestep x CPT consecutive channels each, complex accumulators in
+// registers) and the corrected pixels Dg plus their (l, m, n') are staged in shared memory in
+// chunks and broadcast to every thread: no cross-thread reduction at all.  Phase split as in the
+// gridder (per-timestep FP64 part, FP32 per pixel x channel).
+#include "common.cuh"
+
+namespace idg {
+
+constexpr int kPixChunk = 1024;  // pixels staged per chunk: 48 B each
+
+template <int N, int NT, int CPT>
+__global__ void __launch_bounds__(NT)
+degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
+                 const double *__restrict__ freqs, const float2 *__restrict__ subgrids,
+                 const float4 *__restrict__ aterms, const float *__restrict__ taper,
+                 float4 *__restrict__ vis_out, int32_t T, int32_t C, int32_t n_stations, int32_t L,
+                 double image_size, double w_step) {
+  constexpr int NPIX = N * N;
+  constexpr int CH = NPIX < kPixChunk ? NPIX : kPixChunk;
+  __shared__ float4 s_pix[CH * 2];   // 4 pol complex per pixel
+  __shared__ float4 s_lmn[CH];       // l, m, n', unused
+
+  const int tid = threadIdx.x;
+  const idg_subgrid_meta m = meta[blockIdx.x];
+  const int n_chan = m.n_chan, n_time = m.n_time;
+  const double two_pi = 6.283185307179586476925286766559;
+  const double inv_c0 = 1.0 / kSpeedOfLight;
+  const double u0 = (double)(m.x0 + N / 2 - L / 2) / image_size;
+  const double v0 = (double)(m.y0 + N / 2 - L / 2) / image_size;
+  const double w0 = w_step > 0.0 ? ((double)m.w_index + 0.5) * w_step : 0.0;
+  const double k_mid = 0.5 * (freqs[m.chan_begin] + freqs[m.chan_begin + n_chan - 1]) * inv_c0;
+
+  const int groups = (n_chan + CPT - 1) / CPT;       // channel groups per timestep
+  const int n_items = n_time * groups;
+  const size_t a1_off = ((size_t)m.aterm_slot * n_stations + m.station1) * NPIX;
+  const size_t a2_off = ((size_t)m.aterm_slot * n_stations + m.station2) * NPIX;
+  const float2 *sg = subgrids + (size_t)blockIdx.x * 4 * NPIX;
+
+  for (int item0 = 0; item0 < n_items; item0 += NT) {
+    const int item = item0 + tid;
+    const bool active = item < n_items;
+    const int tl = active ? item / groups : 0;
+    const int cg = active ? (item - tl * groups) * CPT : 0;
+    const float *p = uvw + ((size_t)m.baseline * T + (m.time_begin + tl)) * 3;
+    const float u = p[0], v = p[1], w = p[2];
+    const float bu = (float)(two_pi * ((double)u * k_mid - u0));
+    const float bv = (float)(two_pi * ((double)v * k_mid - v0));
+    const float bw = (float)(two_pi * ((double)w * k_mid - w0));
+    float kd[CPT];
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+      const int cc = min(cg + c, n_chan - 1);
+      kd[c] = (float)(two_pi * (freqs[m.chan_begin + cc] * inv_c0 - k_mid));
+    }
+    float2 acc[CPT][4];
+#pragma unroll
+    for (int c = 0; c < CPT; ++c)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) acc[c][q] = make_float2(0.f, 0.f);
+
+    for (int pix0 = 0; pix0 < NPIX; pix0 += CH) {
+      const int npx = min(CH, NPIX - pix0);
+      __syncthreads();
+      // stage Dg = A1 (taper Ip) A2^H and the pixel coordinates for this chunk
+      for (int i = tid; i < npx; i += NT) {
+        const int pix = pix0 + i;
+        const int y = pix / N, x = pix - y * N;
+        const double l = (double)(x - N / 2) * image_size / (double)N;
+        const double mm = (double)(y - N / 2) * image_size / (double)N;
+        const double r2 = l * l + mm * mm;
+        s_lmn[i] = make_float4((float)l, (float)mm, (float)(-r2 / (1.0 + sqrt(1.0 - r2))), 0.f);
+        const float tp = __ldg(&taper[pix]);
+        float2 p0 = __ldg(&sg[0 * NPIX + pix]), p1 = __ldg(&sg[1 * NPIX + pix]);
+        float2 p2 = __ldg(&sg[2 * NPIX + pix]), p3 = __ldg(&sg[3 * NPIX + pix]);
+        p0.x *= tp; p0.y *= tp; p1.x *= tp; p1.y *= tp;
+        p2.x *= tp; p2.y *= tp; p3.x *= tp; p3.y *= tp;
+        const float4 a01 = __ldg(&aterms[(a1_off + pix) * 2]), a23 = __ldg(&aterms[(a1_off + pix) * 2 + 1]);
+        const float4 b01 = __ldg(&aterms[(a2_off + pix) * 2]), b23 = __ldg(&aterms[(a2_off + pix) * 2 + 1]);
+        const float2 a0 = make_float2(a01.x, a01.y), a1 = make_float2(a01.z, a01.w);
+        const float2 a2 = make_float2(a23.x, a23.y), a3 = make_float2(a23.z, a23.w);
+        const float2 b0 = make_float2(b01.x, b01.y), b1 = make_float2(b01.z, b01.w);
+        const float2 b2 = make_float2(b23.x, b23.y), b3 = make_float2(b23.z, b23.w);
+        // T = A1 P
+        const float2 t00 = cadd(cmul(a0, p0), cmul(a1, p2)), t01 = cadd(cmul(a0, p1), cmul(a1, p3));
+        const float2 t10 = cadd(cmul(a2, p0), cmul(a3, p2)), t11 = cadd(cmul(a2, p1), cmul(a3, p3));
+        // R = T A2^H: (A2^H)[i][j] = conj(A2[j][i])
+        const float2 r0 = cadd(cmul_conj_b(t00, b0), cmul_conj_b(t01, b1));
+        const float2 r1 = cadd(cmul_conj_b(t00, b2), cmul_conj_b(t01, b3));
+        const float2 r2q = cadd(cmul_conj_b(t10, b0), cmul_conj_b(t11, b1));
+        const float2 r3 = cadd(cmul_conj_b(t10, b2), cmul_conj_b(t11, b3));
+        s_pix[2 * i] = make_float4(r0.x, r0.y, r1.x, r1.y);
+        s_pix[2 * i + 1] = make_float4(r2q.x, r2q.y, r3.x, r3.y);
+      }
+      __syncthreads();
+      if (active) {
+#pragma unroll 2
+        for (int i = 0; i < npx; ++i) {
+          const float4 c3 = s_lmn[i];
+          const float4 qa = s_pix[2 * i], qb = s_pix[2 * i + 1];
+          const float pidx = fmaf(u, c3.x, fmaf(v, c3.y, w * c3.z));
+          const float base = fmaf(bu, c3.x, fmaf(bv, c3.y, bw * c3.z));
+#pragma unroll
+          for (int c = 0; c < CPT; ++c) {
+            const float ph = fmaf(pidx, kd[c], base);
+            float s, co;
+            __sincosf(ph, &s, &co);
+            // conjugate phasor: exp(-i ph)
+            cmac(acc[c][0], make_float2(qa.x, qa.y), co, -s);
+            cmac(acc[c][1], make_float2(qa.z, qa.w), co, -s);
+            cmac(acc[c][2], make_float2(qb.x, qb.y), co, -s);
+            cmac(acc[c][3], make_float2(qb.z, qb.w), co, -s);
+          }
+        }
+      }
+    }
+    if (active) {
+      float4 *o = vis_out + (((size_t)m.baseline * T + (m.time_begin + tl)) * C + m.chan_begin + cg) * 2;
+#pragma unroll
+      for (int c = 0; c < CPT; ++c) {
+        if (cg + c < n_chan) {
+          o[2 * c] = make_float4(acc[c][0].x, acc[c][0].y, acc[c][1].x, acc[c][1].y);
+          o[2 * c + 1] = make_float4(acc[c][2].x, acc[c][2].y, acc[c][3].x, acc[c][3].y);
+        }
+      }
+    }
+  }
+}
+
+template <int N, int NT, int CPT>
+static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgrids,
+                    const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream) {
+  degridder_kernel<N, NT, CPT><<<(unsigned)plan->P, NT, 0, stream>>>(
+      plan->meta_dev, uvw, plan->freqs_dev, subgrids, reinterpret_cast<const float4 *>(aterms),
+      taper, reinterpret_cast<float4 *>(vis_out), plan->T, plan->C, plan->n_stations,
+      plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
+  IDG_CUDA_TRY(cudaGetLastError());
+  return IDG_OK;
+}
+
+template <int N>
+static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgrids,
+                    const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream) {
+  // threads own (timestep, CPT channels); pick CPT and the CTA size from the plan's largest block
+  const int mc = plan->max_n_chan;
+  const int cpt = mc >= 4 ? 4 : (mc >= 2 ? 2 : 1);
+  const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
+  const bool small = items <= 128;
+#define IDG_DG(CPT_)                                                                         \
+  return small ? launch_k<N, 128, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream) \
+               : launch_k<N, 256, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream)
+  if (cpt == 4) { IDG_DG(4); }
+  if (cpt == 2) { IDG_DG(2); }
+  IDG_DG(1);
+#undef IDG_DG
+}
+
+int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgrids,
+                     const float2 *aterms, const float *taper, float2 *vis_out,
+                     cudaStream_t stream) {
+  if (plan->P == 0) return IDG_OK;
+  switch (plan->prm.subgrid_size) {
+    case 16: return launch_n<16>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
+    case 24: return launch_n<24>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
+    case 32: return launch_n<32>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
+    case 48: return launch_n<48>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
+    default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
+  }
+}
+
+}  // namespace idg

@@ -1,0 +1,175 @@
+// gridder.cu -- row a1: subgrid images by direct evaluation.
+//
+// Eq. 25, Alg. 1 inner loops, polarised form of section
+// 3.4, one c_p per block:
+//   P[y][x]  = sum_{t,c} Y[b][t][c] exp(+2 pi i (du l_x + dv m_y + dw n'_xy)),   du = u_t f_c/c0 - u0 ...
+//   Sg[y][x] = taper[y][x] A1[y][x]^H P[y][x] A2[y][x]                            (R5)
+//
+// B200 design (not the paper's; the paper gives none): one CTA per subgrid, every thread keeps
+// PPT pixels x 4 polarisations of complex accumulators in registers for the whole block, the
+// visibilities of a batch of timesteps are staged once in shared memory and broadcast to all
+// threads.  FP32 everywhere on the pixel x visibility product; the cancellation-prone part of
+// the phase is taken out per TIMESTEP in FP64 (cost ~ K, not K N^2):
+//   phase(t,c,pix) = pidx(t,pix) * kd_c + base(t,pix)
+//   pidx = u_t l + v_t m + w_t n'            (metres x direction cosine, FP32)
+//   base = bu l + bv m + bw n',  bu = 2 pi (u_t k_mid - u0)  (FP64 -> FP32), k_mid = block centre
+//   kd_c = 2 pi (k_c - k_mid)                (FP64 -> FP32)
+// so that per (visibility, pixel) the work is 1 FMA (phase) + sin/cos.approx (1 FMUL + 2 MUFU) +
+// 16 FMA issued as 8 packed FFMA2.
+#include "common.cuh"
+
+namespace idg {
+
+constexpr int kVisBatch = 256;   // visibilities staged per batch (8 KB)
+constexpr int kMaxChan = 256;    // max channels per subgrid
+
+template <int N, int NT, int PPT>
+__global__ void __launch_bounds__(NT)
+gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
+               const double *__restrict__ freqs, const float4 *__restrict__ vis,
+               const float4 *__restrict__ aterms, const float *__restrict__ taper,
+               float2 *__restrict__ subgrids, int32_t T, int32_t C, int32_t n_stations,
+               int32_t L, double image_size, double w_step) {
+  static_assert(NT * PPT == N * N, "pixels must tile the CTA exactly");
+  __shared__ float4 s_vis[kVisBatch * 2];
+  __shared__ float4 s_t[kVisBatch * 2];
+  __shared__ float s_kd[kMaxChan];
+
+  const int tid = threadIdx.x;
+  const idg_subgrid_meta m = meta[blockIdx.x];
+  const int n_chan = m.n_chan, n_time = m.n_time;
+  const double two_pi = 6.283185307179586476925286766559;
+  const double inv_c0 = 1.0 / kSpeedOfLight;
+  const double u0 = (double)(m.x0 + N / 2 - L / 2) / image_size;
+  const double v0 = (double)(m.y0 + N / 2 - L / 2) / image_size;
+  const double w0 = w_step > 0.0 ? ((double)m.w_index + 0.5) * w_step : 0.0;
+  const double k_mid = 0.5 * (freqs[m.chan_begin] + freqs[m.chan_begin + n_chan - 1]) * inv_c0;
+
+  for (int c = tid; c < n_chan; c += NT)
+    s_kd[c] = (float)(two_pi * (freqs[m.chan_begin + c] * inv_c0 - k_mid));
+
+  // pixel direction cosines (R1: l_x = (x - N/2) S/N; R2: n' = sqrt(1-l^2-m^2) - 1)
+  float pl[PPT], pm[PPT], pn[PPT];
+#pragma unroll
+  for (int k = 0; k < PPT; ++k) {
+    const int pix = tid + k * NT;
+    const int y = pix / N, x = pix - y * N;
+    const double l = (double)(x - N / 2) * image_size / (double)N;
+    const double mm = (double)(y - N / 2) * image_size / (double)N;
+    const double r2 = l * l + mm * mm;
+    pl[k] = (float)l; pm[k] = (float)mm; pn[k] = (float)(-r2 / (1.0 + sqrt(1.0 - r2)));
+  }
+
+  float2 acc[PPT][4];
+#pragma unroll
+  for (int k = 0; k < PPT; ++k)
+#pragma unroll
+    for (int p = 0; p < 4; ++p) acc[k][p] = make_float2(0.f, 0.f);
+
+  const int tb_max = n_chan >= kVisBatch ? 1 : kVisBatch / n_chan;  // timesteps per batch
+  const float *uvw_b = uvw + (size_t)m.baseline * T * 3;
+
+  for (int t0 = 0; t0 < n_time; t0 += tb_max) {
+    const int tb = min(tb_max, n_time - t0);
+    for (int c_lo = 0; c_lo < n_chan; c_lo += kVisBatch) {   // only loops when n_chan > batch
+      const int nc = min(kVisBatch, n_chan - c_lo);
+      __syncthreads();
+      // stage visibilities [tb][nc] (two float4 each) and the per-timestep phase terms
+      for (int i = tid; i < tb * nc * 2; i += NT) {
+        const int tl = i / (2 * nc), r = i - tl * 2 * nc;
+        const size_t g = (((size_t)m.baseline * T + (m.time_begin + t0 + tl)) * C +
+                          (m.chan_begin + c_lo)) * 2 + r;
+        s_vis[i] = __ldg(&vis[g]);
+      }
+      for (int tl = tid; tl < tb; tl += NT) {
+        const float *p = uvw_b + (size_t)(m.time_begin + t0 + tl) * 3;
+        const float u = p[0], v = p[1], w = p[2];
+        s_t[2 * tl] = make_float4(u, v, w, 0.f);
+        s_t[2 * tl + 1] = make_float4((float)(two_pi * ((double)u * k_mid - u0)),
+                                      (float)(two_pi * ((double)v * k_mid - v0)),
+                                      (float)(two_pi * ((double)w * k_mid - w0)), 0.f);
+      }
+      __syncthreads();
+
+      for (int tl = 0; tl < tb; ++tl) {
+        const float4 tu = s_t[2 * tl], tbs = s_t[2 * tl + 1];
+        float pidx[PPT], base[PPT];
+#pragma unroll
+        for (int k = 0; k < PPT; ++k) {
+          pidx[k] = fmaf(tu.x, pl[k], fmaf(tu.y, pm[k], tu.z * pn[k]));
+          base[k] = fmaf(tbs.x, pl[k], fmaf(tbs.y, pm[k], tbs.z * pn[k]));
+        }
+        const float4 *vp = s_vis + (size_t)tl * nc * 2;
+#pragma unroll 2
+        for (int c = 0; c < nc; ++c) {
+          const float kd = s_kd[c_lo + c];
+          const float4 va = vp[2 * c], vb = vp[2 * c + 1];
+#pragma unroll
+          for (int k = 0; k < PPT; ++k) {
+            const float ph = fmaf(pidx[k], kd, base[k]);
+            float s, co;
+            __sincosf(ph, &s, &co);
+            cmac(acc[k][0], make_float2(va.x, va.y), co, s);
+            cmac(acc[k][1], make_float2(va.z, va.w), co, s);
+            cmac(acc[k][2], make_float2(vb.x, vb.y), co, s);
+            cmac(acc[k][3], make_float2(vb.z, vb.w), co, s);
+          }
+        }
+      }
+    }
+  }
+
+  // epilogue: taper * A1^H * P * A2 per pixel, written pol-planar
+  const size_t a1_off = ((size_t)m.aterm_slot * n_stations + m.station1) * (N * N);
+  const size_t a2_off = ((size_t)m.aterm_slot * n_stations + m.station2) * (N * N);
+  float2 *out = subgrids + (size_t)blockIdx.x * 4 * N * N;
+#pragma unroll
+  for (int k = 0; k < PPT; ++k) {
+    const int pix = tid + k * NT;
+    const float4 a01 = __ldg(&aterms[(a1_off + pix) * 2]), a23 = __ldg(&aterms[(a1_off + pix) * 2 + 1]);
+    const float4 b01 = __ldg(&aterms[(a2_off + pix) * 2]), b23 = __ldg(&aterms[(a2_off + pix) * 2 + 1]);
+    const float tp = __ldg(&taper[pix]);
+    const float2 a0 = make_float2(a01.x, a01.y), a1 = make_float2(a01.z, a01.w);
+    const float2 a2 = make_float2(a23.x, a23.y), a3 = make_float2(a23.z, a23.w);
+    const float2 b0 = make_float2(b01.x, b01.y), b1 = make_float2(b01.z, b01.w);
+    const float2 b2 = make_float2(b23.x, b23.y), b3 = make_float2(b23.z, b23.w);
+    const float2 p0 = acc[k][0], p1 = acc[k][1], p2 = acc[k][2], p3 = acc[k][3];
+    const float2 t00 = cadd(cmul_conj_a(a0, p0), cmul_conj_a(a2, p2));
+    const float2 t01 = cadd(cmul_conj_a(a0, p1), cmul_conj_a(a2, p3));
+    const float2 t10 = cadd(cmul_conj_a(a1, p0), cmul_conj_a(a3, p2));
+    const float2 t11 = cadd(cmul_conj_a(a1, p1), cmul_conj_a(a3, p3));
+    float2 r0 = cadd(cmul(t00, b0), cmul(t01, b2));
+    float2 r1 = cadd(cmul(t00, b1), cmul(t01, b3));
+    float2 r2 = cadd(cmul(t10, b0), cmul(t11, b2));
+    float2 r3 = cadd(cmul(t10, b1), cmul(t11, b3));
+    out[0 * N * N + pix] = make_float2(tp * r0.x, tp * r0.y);
+    out[1 * N * N + pix] = make_float2(tp * r1.x, tp * r1.y);
+    out[2 * N * N + pix] = make_float2(tp * r2.x, tp * r2.y);
+    out[3 * N * N + pix] = make_float2(tp * r3.x, tp * r3.y);
+  }
+}
+
+template <int N, int NT, int PPT>
+static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
+                    const float *taper, float2 *subgrids, cudaStream_t stream) {
+  gridder_kernel<N, NT, PPT><<<(unsigned)plan->P, NT, 0, stream>>>(
+      plan->meta_dev, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
+      reinterpret_cast<const float4 *>(aterms), taper, subgrids, plan->T, plan->C,
+      plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
+  IDG_CUDA_TRY(cudaGetLastError());
+  return IDG_OK;
+}
+
+int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
+                   const float *taper, float2 *subgrids, cudaStream_t stream) {
+  if (plan->P == 0) return IDG_OK;
+  switch (plan->prm.subgrid_size) {
+    case 16: return launch_n<16, 64, 4>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 24: return launch_n<24, 192, 3>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 32: return launch_n<32, 256, 4>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 48: return launch_n<48, 384, 6>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
+  }
+}
+
+}  // namespace idg

@@ -1,0 +1,97 @@
+// subgrid_fft.cu -- rows a2 / a5: batched centred 2-D FFT of every subgrid plane, in place.
+//
+// "V_p <- FFT(I_p)" and "I_p <- IFFT(V_p)"; reading R6:
+//   out[b][a] = (1/N^2) sum_{j,i} in[j][i] exp(sign 2 pi i ((a-N/2)(i-N/2) + (b-N/2)(j-N/2))/N)
+// sign = -1 forward, +1 inverse, scale 1/N^2 both ways.  For N = 0 mod 4 (all four sizes) the
+// centred transform is the plain one with checkerboard signs on input and output:
+//   out[a] = (-1)^a FFT((-1)^i in[i]).
+//
+// One CTA per subgrid, one thread per (plane, row): the 32 KB subgrid is brought into shared
+// memory with coalesced 16-byte loads, each thread transforms one row entirely in registers,
+// rows go back to shared memory (pitch N+1 complex: conflict free both ways), each thread then
+// transforms one column and stores it straight to HBM (consecutive threads -> consecutive x).
+// Traffic: one read and one write of the subgrid, 64 N^2 bytes.
+#include "common.cuh"
+#include "fft_codelets.cuh"
+
+namespace idg {
+
+template <int N, bool INV>
+__global__ void __launch_bounds__(4 * N)
+subgrid_fft_kernel(float2 *__restrict__ subgrids) {
+  constexpr int PITCH = N + 1;
+  extern __shared__ float2 sm[];  // [4][N][PITCH]
+  const int tid = threadIdx.x;
+  float2 *sg = subgrids + (size_t)blockIdx.x * 4 * N * N;
+
+  const float4 *in4 = reinterpret_cast<const float4 *>(sg);
+#pragma unroll 4
+  for (int i = tid; i < 2 * N * N; i += 4 * N) {
+    const float4 v = in4[i];
+    const int e = 2 * i;            // complex index in [4][N][N]
+    const int row = e / N, col = e - row * N;   // row runs over plane*N + y
+    sm[row * PITCH + col] = make_float2(v.x, v.y);
+    sm[row * PITCH + col + 1] = make_float2(v.z, v.w);
+  }
+  __syncthreads();
+
+  float2 x[N];
+  {  // row pass: thread = (plane, y)
+    float2 *rowp = sm + tid * PITCH;
+#pragma unroll
+    for (int c = 0; c < N; ++c) {
+      const float2 v = rowp[c];
+      x[c] = (c & 1) ? make_float2(-v.x, -v.y) : v;
+    }
+    fft::Fft<N, INV>::run(x);
+#pragma unroll
+    for (int c = 0; c < N; ++c) rowp[c] = (c & 1) ? make_float2(-x[c].x, -x[c].y) : x[c];
+  }
+  __syncthreads();
+  {  // column pass: thread = (plane, x)
+    const int q = tid / N, c = tid - q * N;
+    const float2 *colp = sm + q * N * PITCH + c;
+#pragma unroll
+    for (int r = 0; r < N; ++r) {
+      const float2 v = colp[r * PITCH];
+      x[r] = (r & 1) ? make_float2(-v.x, -v.y) : v;
+    }
+    fft::Fft<N, INV>::run(x);
+    constexpr float scale = 1.0f / (float)(N * N);
+    float2 *outp = sg + q * N * N + c;
+#pragma unroll
+    for (int r = 0; r < N; ++r) {
+      const float sgn = (r & 1) ? -scale : scale;
+      outp[r * N] = make_float2(x[r].x * sgn, x[r].y * sgn);
+    }
+  }
+}
+
+template <int N>
+static int launch_n(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream) {
+  constexpr size_t smem = sizeof(float2) * 4 * N * (N + 1);
+  if (direction < 0) {
+    IDG_CUDA_TRY(cudaFuncSetAttribute(subgrid_fft_kernel<N, false>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    subgrid_fft_kernel<N, false><<<(unsigned)plan->P, 4 * N, smem, stream>>>(subgrids);
+  } else {
+    IDG_CUDA_TRY(cudaFuncSetAttribute(subgrid_fft_kernel<N, true>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    subgrid_fft_kernel<N, true><<<(unsigned)plan->P, 4 * N, smem, stream>>>(subgrids);
+  }
+  IDG_CUDA_TRY(cudaGetLastError());
+  return IDG_OK;
+}
+
+int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream) {
+  if (plan->P == 0) return IDG_OK;
+  switch (plan->prm.subgrid_size) {
+    case 16: return launch_n<16>(plan, subgrids, direction, stream);
+    case 24: return launch_n<24>(plan, subgrids, direction, stream);
+    case 32: return launch_n<32>(plan, subgrids, direction, stream);
+    case 48: return launch_n<48>(plan, subgrids, direction, stream);
+    default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
+  }
+}
+
+}  // namespace idg
