@@ -16,6 +16,10 @@ namespace idg {
 
 constexpr int kPixChunk = 1024;  // pixels staged per chunk: 48 B each
 
+__device__ __forceinline__ float2 dbc2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 dlo2(float4 v) { return make_float2(v.x, v.y); }
+__device__ __forceinline__ float2 dhi2(float4 v) { return make_float2(v.z, v.w); }
+
 template <int N, int NT, int CPT>
 __global__ void __launch_bounds__(NT)
 degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
@@ -25,7 +29,9 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
                  double image_size, double w_step) {
   constexpr int NPIX = N * N;
   constexpr int CH = NPIX < kPixChunk ? NPIX : kPixChunk;
-  __shared__ float4 s_pix[CH * 2];   // 4 pol complex per pixel
+  // corrected pixels, packed in polarisation pairs like the gridder's visibilities:
+  // (re XX, re XY, re YX, re YY), (im ...) -- one FFMA2 updates two polarisations
+  __shared__ float4 s_pix[CH * 2];
   __shared__ float4 s_lmn[CH];       // l, m, n', unused
 
   const int tid = threadIdx.x;
@@ -60,11 +66,9 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
       const int cc = min(cg + c, n_chan - 1);
       kd[c] = (float)(two_pi * (freqs[m.chan_begin + cc] * inv_c0 - k_mid));
     }
-    float2 acc[CPT][4];
+    float2 re01[CPT], re23[CPT], im01[CPT], im23[CPT];
 #pragma unroll
-    for (int c = 0; c < CPT; ++c)
-#pragma unroll
-      for (int q = 0; q < 4; ++q) acc[c][q] = make_float2(0.f, 0.f);
+    for (int c = 0; c < CPT; ++c) re01[c] = re23[c] = im01[c] = im23[c] = make_float2(0.f, 0.f);
 
     for (int pix0 = 0; pix0 < NPIX; pix0 += CH) {
       const int npx = min(CH, NPIX - pix0);
@@ -96,27 +100,27 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
         const float2 r1 = cadd(cmul_conj_b(t00, b2), cmul_conj_b(t01, b3));
         const float2 r2q = cadd(cmul_conj_b(t10, b0), cmul_conj_b(t11, b1));
         const float2 r3 = cadd(cmul_conj_b(t10, b2), cmul_conj_b(t11, b3));
-        s_pix[2 * i] = make_float4(r0.x, r0.y, r1.x, r1.y);
-        s_pix[2 * i + 1] = make_float4(r2q.x, r2q.y, r3.x, r3.y);
+        s_pix[2 * i] = make_float4(r0.x, r1.x, r2q.x, r3.x);
+        s_pix[2 * i + 1] = make_float4(r0.y, r1.y, r2q.y, r3.y);
       }
       __syncthreads();
       if (active) {
 #pragma unroll 2
         for (int i = 0; i < npx; ++i) {
           const float4 c3 = s_lmn[i];
-          const float4 qa = s_pix[2 * i], qb = s_pix[2 * i + 1];
+          const float4 qr = s_pix[2 * i], qi = s_pix[2 * i + 1];
           const float pidx = fmaf(u, c3.x, fmaf(v, c3.y, w * c3.z));
           const float base = fmaf(bu, c3.x, fmaf(bv, c3.y, bw * c3.z));
 #pragma unroll
           for (int c = 0; c < CPT; ++c) {
-            const float ph = fmaf(pidx, kd[c], base);
             float s, co;
-            __sincosf(ph, &s, &co);
-            // conjugate phasor: exp(-i ph)
-            cmac(acc[c][0], make_float2(qa.x, qa.y), co, -s);
-            cmac(acc[c][1], make_float2(qa.z, qa.w), co, -s);
-            cmac(acc[c][2], make_float2(qb.x, qb.y), co, -s);
-            cmac(acc[c][3], make_float2(qb.z, qb.w), co, -s);
+            __sincosf(fmaf(pidx, kd[c], base), &s, &co);
+            const float ns = -s;
+            // (re + i im) += (qr + i qi)(co - i s): the conjugate phasor of the gridder
+            re01[c] = ffma2(dlo2(qr), dbc2(co), re01[c]); re01[c] = ffma2(dlo2(qi), dbc2(s), re01[c]);
+            re23[c] = ffma2(dhi2(qr), dbc2(co), re23[c]); re23[c] = ffma2(dhi2(qi), dbc2(s), re23[c]);
+            im01[c] = ffma2(dlo2(qi), dbc2(co), im01[c]); im01[c] = ffma2(dlo2(qr), dbc2(ns), im01[c]);
+            im23[c] = ffma2(dhi2(qi), dbc2(co), im23[c]); im23[c] = ffma2(dhi2(qr), dbc2(ns), im23[c]);
           }
         }
       }
@@ -126,8 +130,8 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
 #pragma unroll
       for (int c = 0; c < CPT; ++c) {
         if (cg + c < n_chan) {
-          o[2 * c] = make_float4(acc[c][0].x, acc[c][0].y, acc[c][1].x, acc[c][1].y);
-          o[2 * c + 1] = make_float4(acc[c][2].x, acc[c][2].y, acc[c][3].x, acc[c][3].y);
+          o[2 * c] = make_float4(re01[c].x, im01[c].x, re01[c].y, im01[c].y);
+          o[2 * c + 1] = make_float4(re23[c].x, im23[c].x, re23[c].y, im23[c].y);
         }
       }
     }

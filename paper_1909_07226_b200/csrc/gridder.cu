@@ -16,24 +16,37 @@
 //   kd_c = 2 pi (k_c - k_mid)                (FP64 -> FP32)
 // so that per (visibility, pixel) the work is 1 FMA (phase) + sin/cos.approx (1 FMUL + 2 MUFU) +
 // 16 FMA issued as 8 packed FFMA2.
+//
+// Operand layout of the FFMA2s (measured, profiles/r01_*): the visibilities are re-packed at
+// staging time into polarisation PAIRS, (re XX, re XY, re YX, re YY) and (im ...), so that one
+// FFMA2 is  (acc_pol0, acc_pol1) += (v_pol0, v_pol1) * broadcast(cos or sin)  -- the scalar
+// broadcast and the operand negation are free FFMA2 operand modifiers, which removes the
+// FADD/MOV shuffles a (re, im)-paired accumulator needs.  The accumulators are therefore
+// re[pol pair], im[pol pair] per pixel.
 #include "common.cuh"
 
 namespace idg {
 
-constexpr int kVisBatch = 256;   // visibilities staged per batch (8 KB)
+constexpr int kVisBatch = 256;   // visibilities staged per batch (2 float4 each = 8 KB)
 constexpr int kMaxChan = 256;    // max channels per subgrid
 
-template <int N, int NT, int PPT>
-__global__ void __launch_bounds__(NT)
+__device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
+__device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
+
+template <int N, int NT, int PPT, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
 gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                const double *__restrict__ freqs, const float4 *__restrict__ vis,
                const float4 *__restrict__ aterms, const float *__restrict__ taper,
                float2 *__restrict__ subgrids, int32_t T, int32_t C, int32_t n_stations,
                int32_t L, double image_size, double w_step) {
   static_assert(NT * PPT == N * N, "pixels must tile the CTA exactly");
-  __shared__ float4 s_vis[kVisBatch * 2];
-  __shared__ float4 s_t[kVisBatch * 2];
-  __shared__ float s_kd[kMaxChan];
+  extern __shared__ float4 g_smem[];
+  float4 *s_vis = g_smem;                  // [kVisBatch][2]: (re XX, re XY, re YX, re YY), (im ...)
+  float4 *s_t = s_vis + kVisBatch * 2;     // [kVisBatch][2]: (u, v, w, -), (bu, bv, bw, -)
+  float4 *s_lmn = s_t + kVisBatch * 2;     // [N*N]: (l, m, n', -) per pixel
+  float *s_kd = reinterpret_cast<float *>(s_lmn + N * N);   // [kMaxChan]
 
   const int tid = threadIdx.x;
   const idg_subgrid_meta m = meta[blockIdx.x];
@@ -48,8 +61,8 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
   for (int c = tid; c < n_chan; c += NT)
     s_kd[c] = (float)(two_pi * (freqs[m.chan_begin + c] * inv_c0 - k_mid));
 
-  // pixel direction cosines (R1: l_x = (x - N/2) S/N; R2: n' = sqrt(1-l^2-m^2) - 1)
-  float pl[PPT], pm[PPT], pn[PPT];
+  // pixel direction cosines (R1: l_x = (x - N/2) S/N; R2: n' = sqrt(1-l^2-m^2) - 1), kept in
+  // shared memory: they are needed once per timestep only, not in the channel loop
 #pragma unroll
   for (int k = 0; k < PPT; ++k) {
     const int pix = tid + k * NT;
@@ -57,14 +70,12 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
     const double l = (double)(x - N / 2) * image_size / (double)N;
     const double mm = (double)(y - N / 2) * image_size / (double)N;
     const double r2 = l * l + mm * mm;
-    pl[k] = (float)l; pm[k] = (float)mm; pn[k] = (float)(-r2 / (1.0 + sqrt(1.0 - r2)));
+    s_lmn[pix] = make_float4((float)l, (float)mm, (float)(-r2 / (1.0 + sqrt(1.0 - r2))), 0.f);
   }
 
-  float2 acc[PPT][4];
+  float2 re01[PPT], re23[PPT], im01[PPT], im23[PPT];
 #pragma unroll
-  for (int k = 0; k < PPT; ++k)
-#pragma unroll
-    for (int p = 0; p < 4; ++p) acc[k][p] = make_float2(0.f, 0.f);
+  for (int k = 0; k < PPT; ++k) re01[k] = re23[k] = im01[k] = im23[k] = make_float2(0.f, 0.f);
 
   const int tb_max = n_chan >= kVisBatch ? 1 : kVisBatch / n_chan;  // timesteps per batch
   const float *uvw_b = uvw + (size_t)m.baseline * T * 3;
@@ -74,12 +85,14 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
     for (int c_lo = 0; c_lo < n_chan; c_lo += kVisBatch) {   // only loops when n_chan > batch
       const int nc = min(kVisBatch, n_chan - c_lo);
       __syncthreads();
-      // stage visibilities [tb][nc] (two float4 each) and the per-timestep phase terms
-      for (int i = tid; i < tb * nc * 2; i += NT) {
-        const int tl = i / (2 * nc), r = i - tl * 2 * nc;
+      // stage visibilities [tb][nc], re-packed into polarisation pairs, and the per-timestep terms
+      for (int i = tid; i < tb * nc; i += NT) {
+        const int tl = i / nc, r = i - tl * nc;
         const size_t g = (((size_t)m.baseline * T + (m.time_begin + t0 + tl)) * C +
-                          (m.chan_begin + c_lo)) * 2 + r;
-        s_vis[i] = __ldg(&vis[g]);
+                          (m.chan_begin + c_lo + r)) * 2;
+        const float4 a = __ldg(&vis[g]), b = __ldg(&vis[g + 1]);
+        s_vis[2 * i] = make_float4(a.x, a.z, b.x, b.z);
+        s_vis[2 * i + 1] = make_float4(a.y, a.w, b.y, b.w);
       }
       for (int tl = tid; tl < tb; tl += NT) {
         const float *p = uvw_b + (size_t)(m.time_begin + t0 + tl) * 3;
@@ -96,23 +109,26 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
         float pidx[PPT], base[PPT];
 #pragma unroll
         for (int k = 0; k < PPT; ++k) {
-          pidx[k] = fmaf(tu.x, pl[k], fmaf(tu.y, pm[k], tu.z * pn[k]));
-          base[k] = fmaf(tbs.x, pl[k], fmaf(tbs.y, pm[k], tbs.z * pn[k]));
+          const float4 q = s_lmn[tid + k * NT];
+          pidx[k] = fmaf(tu.x, q.x, fmaf(tu.y, q.y, tu.z * q.z));
+          base[k] = fmaf(tbs.x, q.x, fmaf(tbs.y, q.y, tbs.z * q.z));
         }
         const float4 *vp = s_vis + (size_t)tl * nc * 2;
-#pragma unroll 2
+        const float *kdp = s_kd + c_lo;
+#pragma unroll 4
         for (int c = 0; c < nc; ++c) {
-          const float kd = s_kd[c_lo + c];
-          const float4 va = vp[2 * c], vb = vp[2 * c + 1];
+          const float kd = kdp[c];
+          const float4 vr = vp[2 * c], vi = vp[2 * c + 1];
 #pragma unroll
           for (int k = 0; k < PPT; ++k) {
-            const float ph = fmaf(pidx[k], kd, base[k]);
             float s, co;
-            __sincosf(ph, &s, &co);
-            cmac(acc[k][0], make_float2(va.x, va.y), co, s);
-            cmac(acc[k][1], make_float2(va.z, va.w), co, s);
-            cmac(acc[k][2], make_float2(vb.x, vb.y), co, s);
-            cmac(acc[k][3], make_float2(vb.z, vb.w), co, s);
+            __sincosf(fmaf(pidx[k], kd, base[k]), &s, &co);
+            const float ns = -s;
+            // (re + i im) += (vr + i vi)(co + i s)
+            re01[k] = ffma2(lo2(vr), bc2(co), re01[k]); re01[k] = ffma2(lo2(vi), bc2(ns), re01[k]);
+            re23[k] = ffma2(hi2(vr), bc2(co), re23[k]); re23[k] = ffma2(hi2(vi), bc2(ns), re23[k]);
+            im01[k] = ffma2(lo2(vr), bc2(s), im01[k]);  im01[k] = ffma2(lo2(vi), bc2(co), im01[k]);
+            im23[k] = ffma2(hi2(vr), bc2(s), im23[k]);  im23[k] = ffma2(hi2(vi), bc2(co), im23[k]);
           }
         }
       }
@@ -133,7 +149,8 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
     const float2 a2 = make_float2(a23.x, a23.y), a3 = make_float2(a23.z, a23.w);
     const float2 b0 = make_float2(b01.x, b01.y), b1 = make_float2(b01.z, b01.w);
     const float2 b2 = make_float2(b23.x, b23.y), b3 = make_float2(b23.z, b23.w);
-    const float2 p0 = acc[k][0], p1 = acc[k][1], p2 = acc[k][2], p3 = acc[k][3];
+    const float2 p0 = make_float2(re01[k].x, im01[k].x), p1 = make_float2(re01[k].y, im01[k].y);
+    const float2 p2 = make_float2(re23[k].x, im23[k].x), p3 = make_float2(re23[k].y, im23[k].y);
     const float2 t00 = cadd(cmul_conj_a(a0, p0), cmul_conj_a(a2, p2));
     const float2 t01 = cadd(cmul_conj_a(a0, p1), cmul_conj_a(a2, p3));
     const float2 t10 = cadd(cmul_conj_a(a1, p0), cmul_conj_a(a3, p2));
@@ -149,10 +166,13 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
   }
 }
 
-template <int N, int NT, int PPT>
+template <int N, int NT, int PPT, int MINB>
 static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
                     const float *taper, float2 *subgrids, cudaStream_t stream) {
-  gridder_kernel<N, NT, PPT><<<(unsigned)plan->P, NT, 0, stream>>>(
+  constexpr size_t smem = sizeof(float4) * (kVisBatch * 4 + N * N) + sizeof(float) * kMaxChan;
+  auto kern = gridder_kernel<N, NT, PPT, MINB>;
+  IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<(unsigned)plan->P, NT, smem, stream>>>(
       plan->meta_dev, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
       reinterpret_cast<const float4 *>(aterms), taper, subgrids, plan->T, plan->C,
       plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
@@ -164,10 +184,10 @@ int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, co
                    const float *taper, float2 *subgrids, cudaStream_t stream) {
   if (plan->P == 0) return IDG_OK;
   switch (plan->prm.subgrid_size) {
-    case 16: return launch_n<16, 64, 4>(plan, uvw, vis, aterms, taper, subgrids, stream);
-    case 24: return launch_n<24, 192, 3>(plan, uvw, vis, aterms, taper, subgrids, stream);
-    case 32: return launch_n<32, 256, 4>(plan, uvw, vis, aterms, taper, subgrids, stream);
-    case 48: return launch_n<48, 384, 6>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 16: return launch_n<16, 64, 4, 8>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 24: return launch_n<24, 192, 3, 2>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 32: return launch_n<32, 256, 4, 2>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 48: return launch_n<48, 384, 6, 1>(plan, uvw, vis, aterms, taper, subgrids, stream);
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 }
