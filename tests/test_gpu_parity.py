@@ -184,3 +184,216 @@ def test_grid_and_degrid_end_to_end_tiny(tiny_case):
     idg.idg_degrid(c["plan"], c["wc"].uvw, torch.from_numpy(model).cuda(), c["wc"].aterms, c["wc"].taper, out)
     torch.cuda.synchronize()
     assert H.rel_l2(out.cpu().numpy(), refv) < TOL
+
+
+# ---------------------------------------------------------------------------------------------
+# golden hand-worked plans through the CUDA planner (tests/golden/plan_hand_worked.txt)
+# ---------------------------------------------------------------------------------------------
+
+def test_plan_golden_hand_worked():
+    from tests.test_plan import check_golden_plan, load_golden_plans
+    for name, prm, uvw, f, exp, exp_planned, exp_skipped in load_golden_plans():
+        plan = idg.idg_plan_create(prm, torch.from_numpy(uvw).cuda(), f, np.array([[0, 1]], dtype=np.int32), 2)
+        P, planned, skipped = plan.size()
+        check_golden_plan(plan.metadata(), planned, skipped, exp, exp_planned, exp_skipped)
+
+
+# ---------------------------------------------------------------------------------------------
+# every subgrid size, ragged blocks (odd timestep counts, 1..5 channels, channel counts that are not
+# a multiple of the degridder's per-thread channel group), edge-of-grid subgrids
+# ---------------------------------------------------------------------------------------------
+
+def _ragged_case(N, seed):
+    """A hand-made plan over a small random data set: blocks of odd sizes at random positions."""
+    rng = np.random.default_rng(seed)
+    B, T, C, S, L, n_st = 6, 40, 11, 0.04, 192, 5
+    freqs = 120e6 + 300e3 * np.arange(C)
+    bl = np.array([[i % n_st, (i * 2 + 1) % n_st] for i in range(B)], dtype=np.int32)
+    uvw = (rng.standard_normal((B, T, 3)) * np.array([900.0, 900.0, 60.0])).astype(np.float32)
+    vis = (rng.standard_normal((B, T, C, 4)) + 1j * rng.standard_normal((B, T, C, 4))).astype(np.complex64)
+    n_slots = 3
+    aterms = synth.random_aterms(rng, n_slots, n_st, N)
+    taper = synth.prolate_taper(N)
+    rows = []
+    for b in range(B):
+        t0 = 0
+        while t0 < T:
+            nt = int(min(T - t0, rng.choice([1, 3, 7, 13])))
+            c0 = 0
+            while c0 < C:
+                nc = int(min(C - c0, rng.choice([1, 2, 3, 5])))
+                if rng.random() < 0.85:                      # leave some samples unplanned
+                    k = freqs[c0:c0 + nc].mean() / H.C0
+                    xc = int(np.floor(uvw[b, t0:t0 + nt, 0].mean() * k * S + 0.5)) + int(rng.integers(-2, 3))
+                    yc = int(np.floor(uvw[b, t0:t0 + nt, 1].mean() * k * S + 0.5)) + int(rng.integers(-2, 3))
+                    x0 = int(np.clip(xc + L // 2 - N // 2, 0, L - N))
+                    y0 = int(np.clip(yc + L // 2 - N // 2, 0, L - N))
+                    rows.append((b, bl[b, 0], bl[b, 1], t0, nt, c0, nc, int(rng.integers(0, n_slots)), x0, y0,
+                                 int(rng.integers(-1, 2)), 0))
+                c0 += nc
+            t0 += nt
+    rows[0] = rows[0][:8] + (0, 0) + rows[0][10:]            # corners of the grid
+    rows[1] = rows[1][:8] + (L - N, L - N) + rows[1][10:]
+    meta = np.array(rows, dtype=idg.META_DTYPE)
+    prm = synth.PlanParams(grid_size=L, subgrid_size=N, kernel_size=N // 4, max_timesteps=16, max_channels=8,
+                           aterm_interval=1, flags=0, image_size=S, w_step=3.0)
+    return prm, meta, uvw, freqs, vis, aterms, taper, B, T, n_st
+
+
+@pytest.mark.parametrize("N", [16, 24, 32, 48])
+def test_all_sizes_ragged_blocks_every_stage_and_end_to_end(N):
+    prm, meta, uvw, freqs, vis, aterms, taper, B, T, n_st = _ragged_case(N, 7 + N)
+    plan = idg.idg_plan_from_metadata(prm, meta, freqs, B, T, n_st)
+    P = len(meta)
+    d_uvw, d_vis = torch.from_numpy(uvw).cuda(), torch.from_numpy(vis).cuda()
+    d_at, d_tp = torch.from_numpy(aterms).cuda(), torch.from_numpy(taper).cuda()
+    # gridder
+    ref_img = orc.gridder(prm, meta, uvw, freqs, vis, aterms, taper)
+    sub = torch.zeros((P, 4, N, N), dtype=torch.complex64, device="cuda")
+    idg.idg_gridder(plan, d_uvw, d_vis, d_at, d_tp, sub)
+    torch.cuda.synchronize()
+    got = sub.cpu().numpy()
+    assert max(H.rel_l2(got[p], ref_img[p]) for p in range(P)) < TOL
+    # Alg. 1 end to end
+    L = prm.grid_size
+    ref_grid = orc.grid(prm, meta, uvw, freqs, vis, aterms, taper)
+    g = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    idg.idg_grid(plan, d_uvw, d_vis, d_at, d_tp, g)
+    torch.cuda.synchronize()
+    assert H.rel_l2(g.cpu().numpy(), ref_grid) < TOL
+    # Alg. 2 end to end on a random model grid; unplanned samples must read 0
+    rng = np.random.default_rng(N)
+    model = (rng.standard_normal((4, L, L)) + 1j * rng.standard_normal((4, L, L))).astype(np.complex64)
+    ref_vis = orc.degrid(prm, meta, uvw, freqs, model.astype(np.complex128), aterms, taper, B)
+    out = torch.full(d_vis.shape, 3.0, dtype=torch.complex64, device="cuda")
+    idg.idg_degrid(plan, d_uvw, torch.from_numpy(model).cuda(), d_at, d_tp, out)
+    torch.cuda.synchronize()
+    got_v = out.cpu().numpy()
+    assert H.rel_l2(got_v, ref_vis) < TOL
+    covered = np.zeros(vis.shape[:3], dtype=bool)
+    for r in meta:
+        covered[r["baseline"], r["time_begin"]:r["time_begin"] + r["n_time"],
+                r["chan_begin"]:r["chan_begin"] + r["n_chan"]] = True
+    assert np.all(got_v[~covered] == 0)
+    # per visibility: no planned sample may hide behind the others
+    num = np.linalg.norm((got_v - ref_vis)[covered], axis=-1)
+    den = np.linalg.norm(ref_vis[covered], axis=-1)
+    assert np.max(num / den) < 1e-3
+
+
+def test_empty_plan_is_a_no_op():
+    prm = synth.PlanParams(grid_size=64, subgrid_size=16, kernel_size=4, max_timesteps=4, max_channels=1,
+                           aterm_interval=4, flags=0, image_size=0.01, w_step=0.0)
+    meta = np.zeros(0, dtype=idg.META_DTYPE)
+    plan = idg.idg_plan_from_metadata(prm, meta, np.array([1e8]), 1, 4, 2)
+    assert plan.size() == (0, 0, 4)
+    uvw = torch.zeros((1, 4, 3), device="cuda")
+    vis = torch.ones((1, 4, 1, 4), dtype=torch.complex64, device="cuda")
+    at = torch.from_numpy(synth.identity_aterms(1, 2, 16)).cuda()
+    tp = torch.ones((16, 16), device="cuda")
+    g = torch.ones((4, 64, 64), dtype=torch.complex64, device="cuda")
+    idg.idg_grid(plan, uvw, vis, at, tp, g)
+    idg.idg_degrid(plan, uvw, g, at, tp, vis)
+    torch.cuda.synchronize()
+    assert torch.all(g == 1) and torch.all(vis == 0)
+
+
+def test_everything_skipped_plan():
+    """All samples fall off a tiny grid: the planner emits nothing and counts them."""
+    w = synth.make_workload("tiny")
+    prm = dataclasses.replace(w.params, grid_size=24)
+    plan, wc, meta = _plan_both(w, prm)
+    assert plan.size()[1] + plan.size()[2] == w.B * w.T * w.C
+
+
+# ---------------------------------------------------------------------------------------------
+# the host-buffer entry points (what bench.py's e2e leg times)
+# ---------------------------------------------------------------------------------------------
+
+def test_host_entry_points_match_device_entry_points(tiny_case):
+    c = tiny_case
+    L = c["prm"].grid_size
+    d = c["d"]
+    g_dev = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    idg.idg_grid(c["plan"], c["wc"].uvw, c["wc"].vis, c["wc"].aterms, c["wc"].taper, g_dev)
+    g_host = np.zeros((4, L, L), dtype=np.complex64)
+    idg.idg_grid_host(c["plan"], d["uvw"], d["vis"], d["aterms"], d["taper"], g_host)
+    assert H.rel_l2(g_host, g_dev.cpu().numpy()) < 1e-6
+    v_dev = torch.zeros(c["wc"].vis.shape, dtype=torch.complex64, device="cuda")
+    idg.idg_degrid(c["plan"], c["wc"].uvw, g_dev, c["wc"].aterms, c["wc"].taper, v_dev)
+    v_host = np.zeros(d["vis"].shape, dtype=np.complex64)
+    idg.idg_degrid_host(c["plan"], d["uvw"], g_dev.cpu().numpy(), d["aterms"], d["taper"], v_host)
+    torch.cuda.synchronize()
+    assert np.array_equal(v_host, v_dev.cpu().numpy())
+
+
+# ---------------------------------------------------------------------------------------------
+# full-size configurations in the launch configuration bench.py times: sampled subgrids / samples
+# ---------------------------------------------------------------------------------------------
+
+def _sampled_full_size_check(w, n_sample, seed):
+    plan, wc, meta = _plan_both(w)
+    d = _np(w)
+    P = len(meta)
+    N, L = w.params.subgrid_size, w.params.grid_size
+    rng = np.random.default_rng(seed)
+    pick = np.sort(rng.choice(P, size=min(n_sample, P), replace=False))
+    sample = np.ascontiguousarray(meta[pick])
+    # gridder + FFT on the full plan, compared on the sampled subgrids
+    sub = plan.subgrids()
+    idg.idg_gridder(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, sub)
+    idg.idg_subgrid_fft(plan, sub, -1)
+    torch.cuda.synchronize()
+    got = sub[torch.from_numpy(pick).cuda()].cpu().numpy()
+    ref = orc.subgrid_fft(orc.gridder(w.params, sample, d["uvw"], d["freqs"], d["vis"], d["aterms"], d["taper"]), -1)
+    worst = max(H.rel_l2(got[i], ref[i]) for i in range(len(pick)))
+    assert worst < TOL, worst
+    # adder at full size: property -- the grid total equals the total of all subgrids (per polarisation)
+    g = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    idg.idg_adder(plan, sub, g)
+    torch.cuda.synchronize()
+    tot_sub = sub.to(torch.complex128).sum(dim=(0, 2, 3)).cpu().numpy()
+    tot_grid = g.to(torch.complex128).sum(dim=(1, 2)).cpu().numpy()
+    scale = float(sub.abs().to(torch.float64).sum().item())
+    assert np.max(np.abs(tot_sub - tot_grid)) < 1e-6 * scale
+    # ... and sampled grid windows against the oracle adder restricted to the subgrids that touch them
+    g_np = g.cpu().numpy()
+    sub_np_needed = {}
+    for p in pick[:8]:
+        x0, y0 = int(meta[p]["x0"]), int(meta[p]["y0"])
+        touch = np.nonzero((np.abs(meta["x0"] - x0) < N) & (np.abs(meta["y0"] - y0) < N))[0]
+        acc = np.zeros((4, N, N), dtype=np.complex128)
+        subs = sub[torch.from_numpy(touch).cuda()].cpu().numpy().astype(np.complex128)
+        for s_img, q in zip(subs, touch):
+            dx, dy = int(meta[q]["x0"]) - x0, int(meta[q]["y0"]) - y0
+            xs, ys = max(0, dx), max(0, dy)
+            xe, ye = min(N, N + dx), min(N, N + dy)
+            acc[:, ys:ye, xs:xe] += s_img[:, ys - dy:ye - dy, xs - dx:xe - dx]
+        assert H.rel_l2(g_np[:, y0:y0 + N, x0:x0 + N], acc) < 1e-5
+    # degrid direction: splitter (bit-exact on the sample), then IFFT + degridder on sampled blocks
+    rng2 = np.random.default_rng(seed + 1)
+    model = torch.view_as_complex(torch.randn((4, L, L, 2), device="cuda", generator=torch.Generator("cuda").manual_seed(seed)))
+    out = torch.zeros_like(wc.vis)
+    idg.idg_degrid(plan, wc.uvw, model, wc.aterms, wc.taper, out)
+    torch.cuda.synchronize()
+    model_np = model.cpu().numpy()
+    refv = orc.degrid(w.params, sample, d["uvw"], d["freqs"], model_np.astype(np.complex128), d["aterms"], d["taper"], w.B)
+    got_v = out.cpu().numpy()
+    for r in sample:
+        sl = (int(r["baseline"]), slice(int(r["time_begin"]), int(r["time_begin"] + r["n_time"])),
+              slice(int(r["chan_begin"]), int(r["chan_begin"] + r["n_chan"])))
+        assert H.rel_l2(got_v[sl], refv[sl]) < TOL
+    return P
+
+
+def test_lofar_full_size_sampled():
+    """BASELINE.json configs[1], exactly what bench.py times; 48 sampled subgrids against the oracle."""
+    w = synth.make_workload("lofar")
+    assert _sampled_full_size_check(w, 48, 5) > 4000
+
+
+def test_ska_slice_sampled():
+    """A 600-baseline slice of configs[2]/[3] (long baselines: channel halving, w layers, A-term slots up to
+    31, grid 8192^2): 32 sampled subgrids against the oracle."""
+    w = synth.make_workload("ska", n_baselines=600, baseline_offset=7500)
+    assert _sampled_full_size_check(w, 32, 9) > 15000

@@ -3,6 +3,8 @@ invariants any valid partition has, and against hand-worked tracks whose partiti
 read off without running anything."""
 import dataclasses
 
+import re
+
 import numpy as np
 import pytest
 
@@ -137,3 +139,63 @@ def test_hand_worked_channel_halving():
     assert all((r["station1"], r["station2"]) == (3, 5) for r in meta)
     # centre of the first group: midpoint of 1000 and 1010 px
     assert meta[0]["x0"] == 1005 + 2048 - 8
+
+
+# ---------------------------------------------------------------------------------------------
+# golden fixture: tests/golden/plan_hand_worked.txt (derived by hand from the rule text)
+# ---------------------------------------------------------------------------------------------
+
+def _expand(spec):
+    """'10.3*7' -> 7 copies; '-13+0.9*30' -> arithmetic progression; '60.0*3,0.0*2' -> concatenation;
+    '10.2,10.9' -> literal list."""
+    out = []
+    for part in spec.split(","):
+        part = part.strip()
+        m = re.fullmatch(r"(-?[0-9.]+)\+([0-9.]+)\*(\d+)", part)
+        if m:
+            out += [float(m.group(1)) + float(m.group(2)) * i for i in range(int(m.group(3)))]
+            continue
+        m = re.fullmatch(r"(-?[0-9.]+)\*(\d+)", part)
+        if m:
+            out += [float(m.group(1))] * int(m.group(2))
+            continue
+        out.append(float(part))
+    return np.array(out, dtype=np.float64)
+
+
+def load_golden_plans():
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "plan_hand_worked.txt")
+    cases = []
+    for line in open(path):
+        line = line.strip()
+        if not line.startswith("case "):
+            continue
+        name, over, u, v, w, blocks, planned, skipped = [x.strip() for x in line[5:].split("|")]
+        prm = synth.PlanParams(grid_size=128, subgrid_size=16, kernel_size=4, max_timesteps=100,
+                               max_channels=1, aterm_interval=1000, flags=0, image_size=0.01, w_step=0.0)
+        for kv in over.split():
+            k, val = kv.split("=")
+            prm = dataclasses.replace(prm, **{k: type(getattr(prm, k))(float(val))})
+        f = np.array([150e6])
+        lam = H.C0 / f[0]
+        uvw = np.stack([_expand(u) / prm.image_size * lam, _expand(v) / prm.image_size * lam,
+                        _expand(w) * lam], axis=-1)[None].astype(np.float32)
+        exp = [tuple(int(x) for x in b.strip().split(":")) for b in blocks.split(";")]
+        cases.append((name, prm, uvw, f, exp, int(planned), int(skipped)))
+    return cases
+
+
+def check_golden_plan(meta, planned, skipped, exp, exp_planned, exp_skipped):
+    got = [tuple(int(r[k]) for k in ("time_begin", "n_time", "chan_begin", "n_chan", "aterm_slot", "x0", "y0",
+                                     "w_index")) for r in meta]
+    assert got == exp
+    assert (planned, skipped) == (exp_planned, exp_skipped)
+    assert all(int(r["baseline"]) == 0 and (int(r["station1"]), int(r["station2"])) == (0, 1) for r in meta)
+
+
+@pytest.mark.parametrize("case", load_golden_plans(), ids=lambda c: c[0])
+def test_golden_hand_worked_plans(case):
+    name, prm, uvw, f, exp, exp_planned, exp_skipped = case
+    meta, planned, skipped = orc.plan(prm, uvw, f, np.array([[0, 1]], dtype=np.int32))
+    check_golden_plan(meta, planned, skipped, exp, exp_planned, exp_skipped)
