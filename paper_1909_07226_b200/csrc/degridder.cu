@@ -154,12 +154,16 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
                     const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream) {
   // threads own (timestep, CPT channels); pick CPT and the CTA size from the plan's largest block
   const int mc = plan->max_n_chan;
-  const int cpt = mc >= 4 ? 4 : (mc >= 2 ? 2 : 1);
+  // more channels per thread amortise the per-pixel shared-memory reads and phase set-up, as long as the
+  // largest block still fills a 128-thread CTA
+  int cpt = mc >= 4 ? 4 : (mc >= 2 ? 2 : 1);
+  if (mc >= 8 && plan->max_n_time * ((mc + 7) / 8) >= 128) cpt = 8;
   const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
   const bool small = items <= 128;
 #define IDG_DG(CPT_)                                                                         \
   return small ? launch_k<N, 128, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream) \
                : launch_k<N, 256, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream)
+  if (cpt == 8) { IDG_DG(8); }
   if (cpt == 4) { IDG_DG(4); }
   if (cpt == 2) { IDG_DG(2); }
   IDG_DG(1);
