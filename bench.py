@@ -316,7 +316,16 @@ def run_b200(args):
         pass
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     sub_bytes = 32.0 * N * N * P
-    touched = 2 * 32.0 * min(float(L) * L, float(N) * N * P)
+    # grid pixels covered by at least one subgrid (exact, from the plan metadata): a 2-D difference array
+    # of the subgrid rectangles, summed twice.  Host-side bookkeeping for the byte count only.
+    meta = plan.metadata()
+    diff = np.zeros((L + 1, L + 1), dtype=np.int32)
+    np.add.at(diff, (meta["y0"], meta["x0"]), 1)
+    np.add.at(diff, (meta["y0"] + N, meta["x0"]), -1)
+    np.add.at(diff, (meta["y0"], meta["x0"] + N), -1)
+    np.add.at(diff, (meta["y0"] + N, meta["x0"] + N), 1)
+    touched_px = int(np.count_nonzero(np.cumsum(np.cumsum(diff, axis=0), axis=1)[:L, :L]))
+    touched = 2 * 32.0 * touched_px                      # read + write of every touched 4-pol grid pixel
     extra = {
         "plan_ms": plan_ms, "n_subgrids": P, "n_vis_per_rank": planned, "n_skipped": skipped,
         "stage_ms": stage_ms,
@@ -327,6 +336,10 @@ def run_b200(args):
         "splitter_gbs": (sub_bytes + touched / 2) / (stage_ms["splitter"] * 1e-3) / 1e9,
         "subgrid_fft_gbs": 2 * sub_bytes / (stage_ms["subgrid_fft"] * 1e-3) / 1e9,
         "hbm_peak_gbs": hbm, "hbm_peak_source": "measured" if peaks else "fallback",
+        "touched_grid_pixels": touched_px,
+        "adder_frac_of_hbm": (sub_bytes + touched) / (stage_ms["adder"] * 1e-3) / 1e9 / hbm,
+        "splitter_frac_of_hbm": (sub_bytes + touched / 2) / (stage_ms["splitter"] * 1e-3) / 1e9 / hbm,
+        "subgrid_fft_frac_of_hbm": 2 * sub_bytes / (stage_ms["subgrid_fft"] * 1e-3) / 1e9 / hbm,
     }
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -125,6 +125,13 @@ class Plan:
                "idg_plan_metadata")
         return out
 
+    def slots_needed(self) -> int:
+        """Number of A-term slots the plan indexes (max aterm_slot + 1); cached."""
+        if getattr(self, "_slots", None) is None:
+            meta = self.metadata()
+            self._slots = int(meta["aterm_slot"].max()) + 1 if len(meta) else 0
+        return self._slots
+
     def subgrids(self) -> torch.Tensor:
         """The plan-owned [P][4][N][N] complex64 scratch as a tensor view (not owned by torch)."""
         P = self.size()[0]
@@ -196,9 +203,9 @@ def _shape_check(plan: Plan, uvw=None, vis=None, aterms=None, taper=None, grid=N
         s = tuple(aterms.shape)
         if len(s) != 5 or s[1:] != (plan.n_stations, N, N, 4):
             raise IdgError("aterms shape %s != [slots][%d][%d][%d][4]" % (s, plan.n_stations, N, N))
-        meta = plan.metadata()
-        if len(meta) and int(meta["aterm_slot"].max()) >= s[0]:
-            raise IdgError("aterms has %d slots, the plan needs %d" % (s[0], int(meta["aterm_slot"].max()) + 1))
+        need = plan.slots_needed()
+        if need > s[0]:
+            raise IdgError("aterms has %d slots, the plan needs %d" % (s[0], need))
     if taper is not None and tuple(taper.shape) != (N, N):
         raise IdgError("taper shape %s != (%d, %d)" % (tuple(taper.shape), N, N))
     if grid is not None and tuple(grid.shape) != (4, L, L):

@@ -5,8 +5,9 @@
 // Splitter (Alg. 2): V_p[pol][b][a] = grid[pol][y0+b][x0+a].
 //
 // Subgrids overlap ("subgrids may overlap"), heavily near the uv origin.  Instead
-// of one atomic per subgrid pixel, the plan buckets the subgrids by the 32 x 32 grid tiles they
-// touch (stable in the subgrid index).  One work item = one tile and up to kAdderChunk of its
+// of one atomic per subgrid pixel, the plan buckets the subgrids by the 128 x 8 grid tiles they
+// touch (stable in the subgrid index; wide tiles so that a subgrid row is rarely split between two
+// work items -- a split 32-byte sector is fetched from HBM twice).  One work item = one tile and up to kAdderChunk of its
 // subgrids: the CTA gathers their overlapping parts into registers in plan order and adds the
 // tile to the grid once, with one vector reduction (red.global.add.v2.f32) per pixel.  Every
 // subgrid element is read exactly once; the grid sees one reduction per (work item, pixel)
@@ -24,47 +25,68 @@ __device__ __forceinline__ void red_add_f32x2(float2 *addr, float2 v) {
 
 template <int N>
 __global__ void __launch_bounds__(256)
-adder_kernel(const AdderItem *__restrict__ items, const int32_t *__restrict__ list,
+adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
              const idg_subgrid_meta *__restrict__ meta, const float2 *__restrict__ subgrids,
              float2 *__restrict__ grid, int32_t L) {
-  constexpr int TS = kAdderTile, ROWS = TS / 8;
+  // The tile accumulator lives in shared memory, [pol][row][x].  Warp w owns polarisation w & 3 and
+  // the rows (w >> 2) + 2k of the tile: every (pol, row) slot has exactly one writer, so the
+  // accumulation needs neither atomics nor barriers, and a warp always reads whole subgrid rows
+  // (N consecutive float2: 256 B at N = 32), one lane per pixel.
+  constexpr int TX = kAdderTileX, TY = kAdderTileY, ROWS = TY / 2;
+  constexpr int PASSES = (N + 31) / 32;            // N = 48: a row takes two passes of 32 lanes
+  __shared__ float2 tile[4][TY][TX];
   const AdderItem it = items[blockIdx.x];
-  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-  const int gx = it.tile_x + tx;
-  float2 acc[ROWS][4];
-#pragma unroll
-  for (int k = 0; k < ROWS; ++k)
-#pragma unroll
-    for (int q = 0; q < 4; ++q) acc[k][q] = make_float2(0.f, 0.f);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = warp & 3, r0 = warp >> 2;
+  const int xw = it.x_hi - it.x_lo;                // only the columns this item's subgrids cover
+  for (int i = threadIdx.x; i < 4 * TY * xw; i += 256) tile[i / (TY * xw)][(i / xw) % TY][it.x_lo + i % xw] = make_float2(0.f, 0.f);
+  __syncthreads();
 
-  for (int e = it.begin; e < it.end; ++e) {
-    const int32_t s = __ldg(&list[e]);
-    const int sx = gx - __ldg(&meta[s].x0);
-    const int sy0 = it.tile_y + ty - __ldg(&meta[s].y0);
-    if (sx < 0 || sx >= N) continue;
-    const float2 *sg = subgrids + (size_t)s * 4 * N * N + sx;
+  for (int e0 = it.begin; e0 < it.end; e0 += 2) {   // two subgrids per trip: twice the loads in flight
+    float2 v[2][ROWS][PASSES];
+    int tx0[2];
+    bool ok[2][ROWS];
 #pragma unroll
-    for (int k = 0; k < ROWS; ++k) {
-      const int sy = sy0 + 8 * k;
-      if (sy >= 0 && sy < N) {
+    for (int j = 0; j < 2; ++j) {
+      const bool have = e0 + j < it.end;
+      const int4 ent = have ? __ldg(&list[e0 + j]) : make_int4(0, 0, 0, 0);
+      tx0[j] = ent.y;
+      const int sy0 = r0 - ent.z;
+      const float2 *sg = subgrids + ((size_t)ent.x * 4 + q) * N * N;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const float2 v = __ldg(&sg[(q * N + sy) * N]);
-          acc[k][q].x += v.x; acc[k][q].y += v.y;
+      for (int k = 0; k < ROWS; ++k) {
+        const int sy = sy0 + 2 * k;
+        ok[j][k] = have && sy >= 0 && sy < N;
+#pragma unroll
+        for (int p = 0; p < PASSES; ++p) {
+          const int sx = lane + 32 * p;
+          v[j][k][p] = (ok[j][k] && sx < N) ? __ldg(&sg[sy * N + sx]) : make_float2(0.f, 0.f);
         }
       }
     }
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+#pragma unroll
+      for (int k = 0; k < ROWS; ++k)
+        if (ok[j][k]) {
+#pragma unroll
+          for (int p = 0; p < PASSES; ++p) {
+            const int sx = lane + 32 * p, x = tx0[j] + sx;
+            if (sx < N && x >= 0 && x < TX) {
+              float2 a = tile[q][r0 + 2 * k][x];
+              a.x += v[j][k][p].x; a.y += v[j][k][p].y;
+              tile[q][r0 + 2 * k][x] = a;
+            }
+          }
+        }
   }
-  if (gx < L) {
-#pragma unroll
-    for (int k = 0; k < ROWS; ++k) {
-      const int gy = it.tile_y + ty + 8 * k;
-      if (gy < L) {
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-          red_add_f32x2(&grid[((size_t)q * L + gy) * L + gx], acc[k][q]);
-      }
-    }
+  __syncthreads();
+  // one vector reduction per touched pixel of the tile (untouched ones hold exact zeros and are skipped)
+  for (int i = threadIdx.x; i < 4 * TY * xw; i += 256) {
+    const int x = it.x_lo + i % xw, r = (i / xw) % TY, qq = i / (TY * xw);
+    const float2 a = tile[qq][r][x];
+    const int gx = it.tile_x + x, gy = it.tile_y + r;
+    if ((a.x != 0.f || a.y != 0.f) && gx < L && gy < L) red_add_f32x2(&grid[((size_t)qq * L + gy) * L + gx], a);
   }
 }
 

@@ -25,37 +25,53 @@ static int check_params(const idg_plan_params *p) {
   return IDG_OK;
 }
 
-// Bucket the subgrids by the grid tiles they overlap (stable counting sort in p) and cut every
+// Bucket the subgrids by the 128 x 8 grid tiles they overlap (stable counting sort in p) and cut every
 // tile's list into work items of at most kAdderChunk subgrids.
 static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
-  const int N = pl->prm.subgrid_size, L = pl->prm.grid_size, TS = kAdderTile;
-  const int nt = (L + TS - 1) / TS;
-  std::vector<int64_t> offs((size_t)nt * nt + 1, 0);
+  const int N = pl->prm.subgrid_size, L = pl->prm.grid_size, TX = kAdderTileX, TY = kAdderTileY;
+  const int ntx = (L + TX - 1) / TX, nty = (L + TY - 1) / TY;
+  std::vector<int64_t> offs((size_t)ntx * nty + 1, 0);
   for (const auto &m : pl->meta_host)
-    for (int ty = m.y0 / TS; ty <= (m.y0 + N - 1) / TS; ++ty)
-      for (int tx = m.x0 / TS; tx <= (m.x0 + N - 1) / TS; ++tx) ++offs[(size_t)ty * nt + tx + 1];
+    for (int ty = m.y0 / TY; ty <= (m.y0 + N - 1) / TY; ++ty)
+      for (int tx = m.x0 / TX; tx <= (m.x0 + N - 1) / TX; ++tx) ++offs[(size_t)ty * ntx + tx + 1];
   for (size_t i = 1; i < offs.size(); ++i) offs[i] += offs[i - 1];
   const int64_t total = offs.back();
   std::vector<int32_t> list((size_t)total);
   std::vector<int64_t> cur(offs.begin(), offs.end() - 1);
   for (int64_t p = 0; p < pl->P; ++p) {
     const auto &m = pl->meta_host[(size_t)p];
-    for (int ty = m.y0 / TS; ty <= (m.y0 + N - 1) / TS; ++ty)
-      for (int tx = m.x0 / TS; tx <= (m.x0 + N - 1) / TS; ++tx)
-        list[(size_t)cur[(size_t)ty * nt + tx]++] = (int32_t)p;
+    for (int ty = m.y0 / TY; ty <= (m.y0 + N - 1) / TY; ++ty)
+      for (int tx = m.x0 / TX; tx <= (m.x0 + N - 1) / TX; ++tx)
+        list[(size_t)cur[(size_t)ty * ntx + tx]++] = (int32_t)p;
   }
   std::vector<AdderItem> items;
-  for (int ty = 0; ty < nt; ++ty)
-    for (int tx = 0; tx < nt; ++tx) {
-      const int64_t b = offs[(size_t)ty * nt + tx], e = offs[(size_t)ty * nt + tx + 1];
-      for (int64_t s = b; s < e; s += kAdderChunk)
-        items.push_back(AdderItem{tx * TS, ty * TS, (int32_t)s, (int32_t)std::min<int64_t>(e, s + kAdderChunk)});
+  for (int ty = 0; ty < nty; ++ty)
+    for (int tx = 0; tx < ntx; ++tx) {
+      const int64_t b = offs[(size_t)ty * ntx + tx], e = offs[(size_t)ty * ntx + tx + 1];
+      for (int64_t s = b; s < e; s += kAdderChunk) {
+        const int64_t se = std::min<int64_t>(e, s + kAdderChunk);
+        int lo = TX, hi = 0;
+        for (int64_t i = s; i < se; ++i) {
+          const int x0 = pl->meta_host[(size_t)list[(size_t)i]].x0 - tx * TX;
+          lo = std::min(lo, std::max(0, x0));
+          hi = std::max(hi, std::min(TX, x0 + N));
+        }
+        items.push_back(AdderItem{tx * TX, ty * TY, (int32_t)s, (int32_t)se, lo, hi});
+      }
     }
   pl->n_adder_items = (int64_t)items.size();
   if (total > 0) {
-    IDG_CUDA_TRY(cudaMalloc(&pl->adder_list_dev, sizeof(int32_t) * (size_t)total));
+    // the list entry carries the subgrid's offset relative to its tile: one load per entry in the kernel
+    std::vector<int4> packed((size_t)total);
+    for (int ty = 0; ty < nty; ++ty)
+      for (int tx = 0; tx < ntx; ++tx)
+        for (int64_t i = offs[(size_t)ty * ntx + tx]; i < offs[(size_t)ty * ntx + tx + 1]; ++i) {
+          const auto &m = pl->meta_host[(size_t)list[(size_t)i]];
+          packed[(size_t)i] = make_int4(list[(size_t)i], m.x0 - tx * TX, m.y0 - ty * TY, 0);
+        }
+    IDG_CUDA_TRY(cudaMalloc(&pl->adder_list_dev, sizeof(int4) * (size_t)total));
     IDG_CUDA_TRY(cudaMalloc(&pl->adder_items_dev, sizeof(AdderItem) * items.size()));
-    IDG_CUDA_TRY(cudaMemcpyAsync(pl->adder_list_dev, list.data(), sizeof(int32_t) * (size_t)total,
+    IDG_CUDA_TRY(cudaMemcpyAsync(pl->adder_list_dev, packed.data(), sizeof(int4) * (size_t)total,
                                  cudaMemcpyHostToDevice, stream));
     IDG_CUDA_TRY(cudaMemcpyAsync(pl->adder_items_dev, items.data(), sizeof(AdderItem) * items.size(),
                                  cudaMemcpyHostToDevice, stream));

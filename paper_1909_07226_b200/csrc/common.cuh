@@ -11,12 +11,14 @@
 namespace idg {
 
 constexpr double kSpeedOfLight = 299792458.0;
-constexpr int kAdderTile = 32;        // grid tile edge owned by one adder work item
-constexpr int kAdderChunk = 48;       // max subgrids accumulated by one work item
+constexpr int kAdderTileX = 128;     // grid tile owned by one adder work item: 128 (x) by 8 (y) pixels.  Wide tiles
+constexpr int kAdderTileY = 8;       // keep the subgrid rows (256 B at N = 32) whole: few split 32-byte sectors
+constexpr int kAdderChunk = 64;      // max subgrids accumulated by one work item
 
 struct AdderItem {                    // one unit of adder work: a grid tile and a slice of its list
   int32_t tile_x, tile_y;             // tile origin on the grid (pixels)
   int32_t begin, end;                 // range in adder_list
+  int32_t x_lo, x_hi;                 // tile-local x extent its subgrids cover (zeroed / flushed range)
 };
 
 }  // namespace idg
@@ -31,7 +33,7 @@ struct idg_plan {
   double *freqs_dev = nullptr;        // [C] Hz
   float2 *subgrids_dev = nullptr;     // [P][4][N][N]
   // adder: subgrids bucketed by the grid tiles they overlap (stable in p -> fixed order)
-  int32_t *adder_list_dev = nullptr;  // subgrid indices, grouped by tile
+  int4 *adder_list_dev = nullptr;     // {subgrid index, x0 - tile_x, y0 - tile_y, 0}, grouped by tile
   idg::AdderItem *adder_items_dev = nullptr;
   int64_t n_adder_items = 0;
   // staging for the *_host entry points

@@ -397,3 +397,16 @@ def test_ska_slice_sampled():
     31, grid 8192^2): 32 sampled subgrids against the oracle."""
     w = synth.make_workload("ska", n_baselines=600, baseline_offset=7500)
     assert _sampled_full_size_check(w, 32, 9) > 15000
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs[4]: corners of the kernel sweep (forced blocks), sampled against the oracle
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("N,max_c,max_t,a_int", [(16, 1, 32, 8), (24, 4, 64, 32), (32, 16, 512, 64), (48, 64, 512, 256)])
+def test_sweep_corners_sampled(N, max_c, max_t, a_int):
+    w = synth.make_workload("sweep", n_baselines=12, n_time=512, subgrid_size=N, max_channels=max_c,
+                            max_timesteps=max_t, aterm_interval=a_int)
+    P = _sampled_full_size_check(w, 6, 100 + N)
+    eff_t = min(max_t, a_int)
+    assert P == 12 * (512 // eff_t) * (64 // max_c)
