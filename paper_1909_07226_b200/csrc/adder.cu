@@ -59,8 +59,8 @@ adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
         ok[j][k] = have && sy >= 0 && sy < N;
 #pragma unroll
         for (int p = 0; p < PASSES; ++p) {
-          const int sx = lane + 32 * p;
-          v[j][k][p] = (ok[j][k] && sx < N) ? __ldg(&sg[sy * N + sx]) : make_float2(0.f, 0.f);
+          const int sx = lane + 32 * p, x = tx0[j] + sx;    // lanes outside the tile do not load
+          v[j][k][p] = (ok[j][k] && sx < N && x >= 0 && x < TX) ? __ldg(&sg[sy * N + sx]) : make_float2(0.f, 0.f);
         }
       }
     }

@@ -44,12 +44,15 @@ static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
       for (int tx = m.x0 / TX; tx <= (m.x0 + N - 1) / TX; ++tx)
         list[(size_t)cur[(size_t)ty * ntx + tx]++] = (int32_t)p;
   }
+  // work items of at most `chunk` subgrids: kAdderChunk when there is plenty of work, shorter lists on small
+  // plans so that the items still fill the GPU (a few per resident CTA slot)
+  const int64_t chunk = std::max<int64_t>(8, std::min<int64_t>(kAdderChunk, total / 4096));
   std::vector<AdderItem> items;
   for (int ty = 0; ty < nty; ++ty)
     for (int tx = 0; tx < ntx; ++tx) {
       const int64_t b = offs[(size_t)ty * ntx + tx], e = offs[(size_t)ty * ntx + tx + 1];
-      for (int64_t s = b; s < e; s += kAdderChunk) {
-        const int64_t se = std::min<int64_t>(e, s + kAdderChunk);
+      for (int64_t s = b; s < e; s += chunk) {
+        const int64_t se = std::min<int64_t>(e, s + chunk);
         int lo = TX, hi = 0;
         for (int64_t i = s; i < se; ++i) {
           const int x0 = pl->meta_host[(size_t)list[(size_t)i]].x0 - tx * TX;
