@@ -105,7 +105,7 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
       }
       __syncthreads();
       if (active) {
-#pragma unroll 2
+#pragma unroll(CPT >= 8 ? 1 : 2)
         for (int i = 0; i < npx; ++i) {
           const float4 c3 = s_lmn[i];
           const float4 qr = s_pix[2 * i], qi = s_pix[2 * i + 1];
