@@ -185,7 +185,7 @@ int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, co
   if (plan->P == 0) return IDG_OK;
   switch (plan->prm.subgrid_size) {
     case 16: return launch_n<16, 64, 4, 8>(plan, uvw, vis, aterms, taper, subgrids, stream);
-    case 24: return launch_n<24, 192, 3, 2>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 24: return launch_n<24, 96, 6, 5>(plan, uvw, vis, aterms, taper, subgrids, stream);
     case 32: return launch_n<32, 256, 4, 2>(plan, uvw, vis, aterms, taper, subgrids, stream);
     case 48: return launch_n<48, 384, 6, 1>(plan, uvw, vis, aterms, taper, subgrids, stream);
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
