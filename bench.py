@@ -34,6 +34,9 @@ N_SM, FP32_LANES, SM_MAX_HZ = 148, 128, 1.965e9
 # (visibility, pixel); expressed in FLOP-equivalents at 2 per lane-op against 2*lanes*clock.
 LANE_OPS_PER_VIS_PIXEL = 18
 ALU_PEAK_TFLOPS = N_SM * FP32_LANES * 2 * SM_MAX_HZ / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of one gridder launch from the committed ncu --set full capture
+# (profiles/r01_final_ncu_summary.md); only the workload that was captured has a number
+NCU_TRAFFIC_BYTES = {"lofar": 159508992 + 107927296}
 
 
 def parse_args():
@@ -303,7 +306,7 @@ def run_b200(args):
     flop_equiv = 2.0 * LANE_OPS_PER_VIS_PIXEL * vis_pixels
     ach = flop_equiv / (stage_ms["gridder"] * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "gridder_kernel", "achieved": ach, "peak": ALU_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS, "traffic": None,
+                "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
                 "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1965 MHz (DESIGN.md), not in MEASURED_PEAKS.json",
                 "work": "18 FP32 lane-ops (17 FMA + 1 FMUL) per (visibility, pixel), 2 FLOP-equivalents each"}
     if clocks.get("sm_mhz"):
