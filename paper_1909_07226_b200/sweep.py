@@ -46,7 +46,7 @@ def points(quick: bool):
             pts.append((N, c, 128, 256))
         for t in (32, 64, 256, 512):
             pts.append((N, 16, t, 512))
-        for a in (8, 32, 64):
+        for a in (8, 16):                      # A-term interval below the timestep limit: it caps the block
             pts.append((N, 16, 512, a))
     if quick:
         pts = [p for p in pts if p[0] in (16, 32)][::3]
