@@ -143,6 +143,22 @@ int idg_degridder(const idg_plan *plan, const float *uvw_dev, const void *subgri
                   const void *aterms_dev, const float *taper_dev, void *vis_out_dev,
                   void *cuda_stream);
 
+/* ---- image-plane side of W-stacking (OUTSIDE the timed hot path) --------------
+ * Alg. 1 last line "I <- FFT(V) / c-bar" (R8) and Alg. 2 first lines with the
+ * per-subgrid w offset w0 = (w_index + 0.5) w_step (R4) resolved by W-stacking:
+ * one grid per w layer; its image lacks exp(+2 pi i w0 n'(l, m)), l_x = (x - L/2) S / L (Eq. 5),
+ * n' = sqrt(1 - l^2 - m^2) - 1 (R2).  The large FFT is the caller's (library).  Images are [4][L][L] complex64,
+ * device; asynchronous on cuda_stream.  sign = +1 imaging, -1 prediction.
+ *   idg_image_w_accumulate: acc += layer * exp(sign 2 pi i w0 n')
+ *   idg_image_w_apply:      out  = in    * exp(sign 2 pi i w0 n')   (out may alias in)
+ *   idg_image_divide:       image[pol][y][x] /= cbar[y][x], cbar [L][L] float32 (the image-domain taper c-bar)
+ * Errors: IDG_ERR_INVALID_ARG, IDG_ERR_CUDA. */
+int idg_image_w_accumulate(void *acc_dev, const void *layer_dev, int32_t L, double image_size, double w0,
+                           int32_t sign, void *cuda_stream);
+int idg_image_w_apply(void *out_dev, const void *in_dev, int32_t L, double image_size, double w0, int32_t sign,
+                      void *cuda_stream);
+int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

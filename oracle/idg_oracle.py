@@ -2,9 +2,11 @@
 
 TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and
 bench.py's cpu_baseline / --impl reference legs.  It imports nothing from the
-product package and the product never imports it.  All arithmetic lives in
-idg_oracle.c; this file only marshals numpy arrays (and composes the stages in
-the order of Alg. 1 / Alg. 2).
+product package and the product never imports it.  The arithmetic of the hot path lives in
+idg_oracle.c; this file marshals numpy arrays and composes the stages in
+the order of Alg. 1 / Alg. 2.  The image-plane wrap with
+W-stacking at the end of the file (NEXT-1, outside the timed path) is plain numpy.
+Pins of that part: tests/test_imaging_pins.py (Eq. 11 and Eq. 6 with the full w term).
 """
 from __future__ import annotations
 
@@ -177,3 +179,71 @@ def degrid(params, meta, uvw, freqs, grid_in, aterms, taper, n_baselines: int) -
     sub = splitter(meta, grid_in, int(params.subgrid_size))
     img = subgrid_fft(sub, +1)
     return degridder(params, meta, uvw, freqs, img, aterms, taper, n_baselines)
+
+
+# ---- image-plane wrap with W-stacking (outside the timed path) --------------
+# Alg. 1 last line "I <- FFT(V)/c-bar" (reading R8: inverse-sign centred DFT, unnormalised),
+# Alg. 2 first lines "I <- I/c-bar; V <- FFT(I)", the per-subgrid w offset of Alg. 1
+# (R4) resolved per w layer (W-stacking).  Plain numpy, float64; the library FFT
+# with its centring shifts is the step, everything else is written out.
+
+def _centred_ifft2_unnormalised(grid: np.ndarray) -> np.ndarray:
+    L = grid.shape[-1]
+    return np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(grid, axes=(-2, -1))), axes=(-2, -1)) * (L * L)
+
+
+def _centred_fft2(img: np.ndarray) -> np.ndarray:
+    return np.fft.fftshift(np.fft.fft2(np.fft.ifftshift(img, axes=(-2, -1))), axes=(-2, -1))
+
+
+def image_nprime(L: int, image_size: float) -> np.ndarray:
+    """n'(l_x, m_y) on the image raster, l_x = (x - L/2) S / L (Eq. 5; R2)."""
+    l = (np.arange(L, dtype=np.float64) - L // 2) * image_size / L
+    ll, mm = np.meshgrid(l, l)
+    r2 = ll * ll + mm * mm
+    return -r2 / (1.0 + np.sqrt(1.0 - r2))
+
+
+def image_taper(taper: np.ndarray, L: int) -> np.ndarray:
+    """c-bar [L][L]: the subgrid taper [N][N] carried to the image raster.  Section 4.2: the
+    effective window is the trigonometric interpolation of the discrete one, i.e. its centred DFT
+    coefficients evaluated on the finer raster."""
+    t = np.asarray(taper, dtype=np.float64)
+    N = t.shape[0]
+    k = np.arange(N) - N // 2
+    F = np.exp(-2j * np.pi * np.outer(k, k) / N) / N            # centred DFT, scale 1/N per axis
+    coef = F @ t @ F.T                                          # [N][N] coefficients
+    x = np.arange(L) - L // 2
+    E = np.exp(2j * np.pi * np.outer(x, k) / L)                 # evaluate on the L-raster
+    return np.real(E @ coef @ E.T)
+
+
+def w_layers(meta: np.ndarray):
+    return [int(w) for w in np.unique(meta["w_index"])]
+
+
+def dirty_image(params, meta, uvw, freqs, vis, aterms, taper) -> np.ndarray:
+    """Alg. 1 complete, one grid per w layer: image[pol][y][x] = (sum_layers IDFT(grid_layer) e^{+2 pi i w0 n'}) / c-bar."""
+    L, S = int(params.grid_size), float(params.image_size)
+    n = image_nprime(L, S)
+    img = np.zeros((4, L, L), dtype=np.complex128)
+    for wi in w_layers(meta):
+        sel = np.ascontiguousarray(meta[meta["w_index"] == wi])
+        g = grid(params, sel, uvw, freqs, vis, aterms, taper)
+        w0 = (wi + 0.5) * params.w_step if params.w_step > 0 else 0.0
+        img += _centred_ifft2_unnormalised(g) * np.exp(2j * np.pi * w0 * n)
+    return img / image_taper(taper, L)
+
+
+def predict(params, meta, uvw, freqs, image, aterms, taper, n_baselines: int) -> np.ndarray:
+    """Alg. 2 complete: per w layer, V = FFT((I / c-bar) e^{-2 pi i w0 n'}), then splitter -> IFFT -> degridder."""
+    L, S = int(params.grid_size), float(params.image_size)
+    n = image_nprime(L, S)
+    base = np.asarray(image, dtype=np.complex128) / image_taper(taper, L)
+    out = np.zeros((n_baselines, np.asarray(uvw).shape[1], len(freqs), 4), dtype=np.complex128)
+    for wi in w_layers(meta):
+        sel = np.ascontiguousarray(meta[meta["w_index"] == wi])
+        w0 = (wi + 0.5) * params.w_step if params.w_step > 0 else 0.0
+        g = _centred_fft2(base * np.exp(-2j * np.pi * w0 * n))
+        out += degrid(params, sel, uvw, freqs, g, aterms, taper, n_baselines)   # layers cover disjoint samples
+    return out

@@ -25,7 +25,8 @@ EXPORTS = (
     "idg_strerror", "idg_last_cuda_error", "idg_plan_create", "idg_plan_from_metadata",
     "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
-    "idg_adder", "idg_splitter", "idg_degridder")
+    "idg_adder", "idg_splitter", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
+    "idg_image_divide")
 
 
 class IdgError(RuntimeError):
@@ -292,3 +293,30 @@ def idg_degrid_host(plan: Plan, uvw, grid, aterms, taper, vis_out, stream=None) 
         raise IdgError("vis_out must be a contiguous complex64 array (it is written in place)")
     _check(lib().idg_degrid_host(plan.handle, up, gp, ap, ctypes.c_int32(int(aterms.shape[0])), tp, vp,
                                  _stream(stream)), "idg_degrid_host")
+
+
+def idg_image_w_accumulate(acc, layer, image_size: float, w0: float, sign: int = 1, stream=None) -> None:
+    """acc += layer * exp(sign 2 pi i w0 n'(l, m)); [4][L][L] complex64 device tensors (W-stacking)."""
+    L = int(acc.shape[-1])
+    if tuple(acc.shape) != (4, L, L) or tuple(layer.shape) != (4, L, L):
+        raise IdgError("images must be [4][L][L]")
+    _check(lib().idg_image_w_accumulate(_dev(acc, _C64, "acc"), _dev(layer, _C64, "layer"), ctypes.c_int32(L),
+                                        ctypes.c_double(image_size), ctypes.c_double(w0), ctypes.c_int32(sign),
+                                        _stream(stream)), "idg_image_w_accumulate")
+
+
+def idg_image_w_apply(out, inp, image_size: float, w0: float, sign: int, stream=None) -> None:
+    L = int(out.shape[-1])
+    if tuple(out.shape) != (4, L, L) or tuple(inp.shape) != (4, L, L):
+        raise IdgError("images must be [4][L][L]")
+    _check(lib().idg_image_w_apply(_dev(out, _C64, "out"), _dev(inp, _C64, "in"), ctypes.c_int32(L),
+                                   ctypes.c_double(image_size), ctypes.c_double(w0), ctypes.c_int32(sign),
+                                   _stream(stream)), "idg_image_w_apply")
+
+
+def idg_image_divide(image, cbar, stream=None) -> None:
+    L = int(image.shape[-1])
+    if tuple(image.shape) != (4, L, L) or tuple(cbar.shape) != (L, L):
+        raise IdgError("image must be [4][L][L] and cbar [L][L]")
+    _check(lib().idg_image_divide(_dev(image, _C64, "image"), _dev(cbar, _F32, "cbar"), ctypes.c_int32(L),
+                                  _stream(stream)), "idg_image_divide")

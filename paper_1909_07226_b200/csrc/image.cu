@@ -1,0 +1,95 @@
+// image.cu -- image-plane side of W-stacking (NEXT-1 row of SURVEY.md section 8f; outside the timed hot path).
+//
+// Alg. 1 last line, "I <- FFT(V) / c-bar" (R8), and Alg. 2 first lines, "I <- I / c-bar;
+// V <- FFT(I)", with the w-offset w0p of every subgrid (Alg. 1, R4) resolved by
+// W-stacking (mentioned PAPER.md:166): the subgrids of one w layer are gridded with phasors that carry
+// (w - w0) n', so the layer's image lacks exp(+2 pi i w0 n'(l, m)); multiplying it back per layer and summing
+// the layers gives the image of Eq. 11.  Prediction applies the conjugate factor before the
+// layer's forward transform.  The large FFT itself is the library's (cuFFT through torch.fft).
+//
+//   idg_image_w_accumulate:  acc[pol][y][x] += layer[pol][y][x] * exp(sign 2 pi i w0 n'(l_x, m_y)),
+//                            l_x = (x - L/2) S / L  (Eq. 5), n' = sqrt(1 - l^2 - m^2) - 1 (R2)
+//   idg_image_w_apply:       out = in * exp(sign 2 pi i w0 n')            (prediction direction)
+//   idg_image_divide:        image[pol][y][x] /= cbar[y][x]               (c-bar: image-domain taper)
+#include "common.cuh"
+
+namespace idg {
+
+__device__ __forceinline__ float2 w_phasor(int x, int y, int L, double image_size, double w0, double sign) {
+  // FP64 phase: w0 n' reaches thousands of radians at the image edge for large w layers
+  const double l = (double)(x - L / 2) * image_size / (double)L;
+  const double m = (double)(y - L / 2) * image_size / (double)L;
+  const double r2 = l * l + m * m;
+  const double n = -r2 / (1.0 + sqrt(1.0 - r2));
+  double s, c;
+  sincospi(2.0 * sign * w0 * n, &s, &c);
+  return make_float2((float)c, (float)s);
+}
+
+template <bool ACCUMULATE>
+__global__ void __launch_bounds__(256)
+image_w_kernel(float2 *__restrict__ dst, const float2 *__restrict__ src, int L, double image_size,
+               double w0, double sign) {
+  const int x = blockIdx.x * 64 + (threadIdx.x & 63);
+  const int y = blockIdx.y * 4 + (threadIdx.x >> 6);
+  if (x >= L || y >= L) return;
+  const float2 ph = w_phasor(x, y, L, image_size, w0, sign);   // one phasor serves the four polarisations
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const size_t i = ((size_t)q * L + y) * L + x;
+    const float2 v = cmul(src[i], ph);
+    if (ACCUMULATE) { float2 a = dst[i]; a.x += v.x; a.y += v.y; dst[i] = a; }
+    else dst[i] = v;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+image_divide_kernel(float2 *__restrict__ image, const float *__restrict__ cbar, int L) {
+  const int x = blockIdx.x * 64 + (threadIdx.x & 63);
+  const int y = blockIdx.y * 4 + (threadIdx.x >> 6);
+  if (x >= L || y >= L) return;
+  const float inv = 1.0f / cbar[(size_t)y * L + x];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const size_t i = ((size_t)q * L + y) * L + x;
+    float2 v = image[i];
+    v.x *= inv; v.y *= inv;
+    image[i] = v;
+  }
+}
+
+}  // namespace idg
+
+using namespace idg;
+
+extern "C" {
+
+int idg_image_w_accumulate(void *acc_dev, const void *layer_dev, int32_t L, double image_size, double w0,
+                           int32_t sign, void *stream) {
+  if (!acc_dev || !layer_dev || L < 1 || !(image_size > 0.0) || (sign != 1 && sign != -1)) return IDG_ERR_INVALID_ARG;
+  const dim3 grid((L + 63) / 64, (L + 3) / 4);
+  image_w_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>((float2 *)acc_dev, (const float2 *)layer_dev, L,
+                                                              image_size, w0, (double)sign);
+  IDG_CUDA_TRY(cudaGetLastError());
+  return IDG_OK;
+}
+
+int idg_image_w_apply(void *out_dev, const void *in_dev, int32_t L, double image_size, double w0, int32_t sign,
+                      void *stream) {
+  if (!out_dev || !in_dev || L < 1 || !(image_size > 0.0) || (sign != 1 && sign != -1)) return IDG_ERR_INVALID_ARG;
+  const dim3 grid((L + 63) / 64, (L + 3) / 4);
+  image_w_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>((float2 *)out_dev, (const float2 *)in_dev, L,
+                                                               image_size, w0, (double)sign);
+  IDG_CUDA_TRY(cudaGetLastError());
+  return IDG_OK;
+}
+
+int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *stream) {
+  if (!image_dev || !cbar_dev || L < 1) return IDG_ERR_INVALID_ARG;
+  const dim3 grid((L + 63) / 64, (L + 3) / 4);
+  image_divide_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((float2 *)image_dev, cbar_dev, L);
+  IDG_CUDA_TRY(cudaGetLastError());
+  return IDG_OK;
+}
+
+}  // extern "C"

@@ -410,3 +410,35 @@ def test_sweep_corners_sampled(N, max_c, max_t, a_int):
     P = _sampled_full_size_check(w, 6, 100 + N)
     eff_t = min(max_t, a_int)
     assert P == 12 * (512 // eff_t) * (64 // max_c)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: image-plane wrap with W-stacking (paper_1909_07226_b200.imaging) against the oracle
+# ---------------------------------------------------------------------------------------------
+
+def test_w_stacked_dirty_image_and_prediction():
+    from paper_1909_07226_b200 import imaging
+    w = synth.make_workload("tiny")
+    prm = dataclasses.replace(w.params, w_step=150.0)
+    wc = _cuda(w)
+    d = _np(w)
+    meta, _, _ = orc.plan(prm, d["uvw"], d["freqs"], w.baselines)
+    assert len(orc.w_layers(meta)) >= 3
+    ref_img = orc.dirty_image(prm, meta, d["uvw"], d["freqs"], d["vis"], d["aterms"], d["taper"])
+    img = imaging.dirty_image(prm, wc.uvw, w.freqs, w.baselines, w.n_stations, wc.vis, wc.aterms, wc.taper)
+    L = prm.grid_size
+    inner = slice(L // 8, 7 * L // 8)                     # c-bar is tiny at the very edge: compare where it is not
+    assert H.rel_l2(img.cpu().numpy()[:, inner, inner], ref_img[:, inner, inner]) < TOL
+    # c-bar itself
+    cb = imaging.image_taper(wc.taper, L).cpu().numpy()
+    assert H.rel_l2(cb, orc.image_taper(d["taper"], L)) < 1e-6
+    # prediction from a model image of a few sources
+    rng = np.random.default_rng(3)
+    model = np.zeros((4, L, L), dtype=np.complex64)
+    for _ in range(5):
+        x, y = rng.integers(L // 4, 3 * L // 4, 2)
+        model[0, y, x] = model[3, y, x] = rng.uniform(0.5, 2.0)
+    ref_vis = orc.predict(prm, meta, d["uvw"], d["freqs"], model.astype(np.complex128), d["aterms"], d["taper"], w.B)
+    got = imaging.predict(prm, wc.uvw, w.freqs, w.baselines, w.n_stations, torch.from_numpy(model).cuda(),
+                          wc.aterms, wc.taper, w.C)
+    assert H.rel_l2(got.cpu().numpy(), ref_vis) < TOL
