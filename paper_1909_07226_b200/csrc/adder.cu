@@ -122,11 +122,13 @@ int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cud
 }
 
 int launch_splitter(const idg_plan *plan, const float2 *grid, float2 *subgrids,
-                    cudaStream_t stream) {
-  if (plan->P == 0) return IDG_OK;
-  const unsigned nb = (unsigned)plan->P;
+                    cudaStream_t stream, int64_t p0, int64_t np) {
+  if (np < 0) np = plan->P - p0;
+  if (np <= 0) return IDG_OK;
+  const unsigned nb = (unsigned)np;
+  subgrids += (size_t)p0 * 4 * plan->prm.subgrid_size * plan->prm.subgrid_size;
   const int32_t L = plan->prm.grid_size;
-#define IDG_SPL(N_) splitter_kernel<N_><<<nb, 256, 0, stream>>>(plan->meta_dev, grid, subgrids, L)
+#define IDG_SPL(N_) splitter_kernel<N_><<<nb, 256, 0, stream>>>(plan->meta_dev + p0, grid, subgrids, L)
   switch (plan->prm.subgrid_size) {
     case 16: IDG_SPL(16); break;
     case 24: IDG_SPL(24); break;

@@ -127,6 +127,9 @@ void idg_plan_destroy(idg_plan *pl) {
   cudaFree(pl->adder_list_dev); cudaFree(pl->adder_items_dev);
   cudaFree(pl->h_uvw_dev); cudaFree(pl->h_vis_dev); cudaFree(pl->h_aterms_dev);
   cudaFree(pl->h_grid_dev); cudaFree(pl->h_taper_dev);
+  if (pl->h_copy_stream) cudaStreamDestroy(pl->h_copy_stream);
+  for (auto e : pl->h_ev_in) if (e) cudaEventDestroy(e);
+  for (auto e : pl->h_ev_out) if (e) cudaEventDestroy(e);
   delete pl;
 }
 

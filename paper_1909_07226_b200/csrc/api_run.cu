@@ -1,5 +1,8 @@
 // api_run.cu -- the compute entry points of include/idg_b200.h (stage calls, Alg. 1, Alg. 2,
 // and the host-buffer variants).  Every step runs in the kernels of this library.
+#include <algorithm>
+#include <vector>
+
 #include "common.cuh"
 
 using namespace idg;
@@ -100,22 +103,76 @@ int idg_degrid(const idg_plan *pl, const float *uvw_dev, const void *grid_dev,
   return rc;
 }
 
+// The host-buffer calls overlap the PCIe copies with the kernels: the baselines are cut into kHostChunks
+// contiguous ranges (the metadata is sorted by baseline, so a range of baselines is a range of subgrids and a
+// contiguous slice of vis); uploads run on the plan's copy stream, kernels on the caller's stream, events
+// order them.  Gridding: chunk k is gridded while chunk k+1 and then the grid itself are uploaded; the adder
+// runs once at the end.  Degridding: chunk k's visibilities travel back while chunk k+1 is predicted.
+struct HostChunk { int32_t b0, b1; int64_t p0, p1; };
+
+static int ensure_host_pipeline(idg_plan *pl) {
+  if (!pl->h_copy_stream) IDG_CUDA_TRY(cudaStreamCreateWithFlags(&pl->h_copy_stream, cudaStreamNonBlocking));
+  for (auto &e : pl->h_ev_in) if (!e) IDG_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  for (auto &e : pl->h_ev_out) if (!e) IDG_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  return IDG_OK;
+}
+
+static std::vector<HostChunk> host_chunks(const idg_plan *pl) {
+  std::vector<HostChunk> out;
+  const int n = std::min<int>(idg_plan::kHostChunks, pl->B);
+  int64_t p = 0;
+  for (int k = 0; k < n; ++k) {
+    HostChunk c;
+    c.b0 = (int32_t)((int64_t)pl->B * k / n);
+    c.b1 = (int32_t)((int64_t)pl->B * (k + 1) / n);
+    c.p0 = p;
+    while (p < pl->P && pl->meta_host[(size_t)p].baseline < c.b1) ++p;
+    c.p1 = p;
+    out.push_back(c);
+  }
+  return out;
+}
+
 int idg_grid_host(idg_plan *pl, const float *uvw_host, const void *vis_host,
                   const void *aterms_host, int32_t n_slots, const float *taper_host,
                   void *grid_host, void *stream) {
   if (!pl || !uvw_host || !vis_host || !aterms_host || !taper_host || !grid_host) return IDG_ERR_INVALID_ARG;
   if (n_slots < needed_slots(pl)) return IDG_ERR_PLAN_MISMATCH;
   int rc = ensure_staging(pl, n_slots);
+  if (rc == IDG_OK) rc = ensure_host_pipeline(pl);
   if (rc != IDG_OK) return rc;
   const size_t N = pl->prm.subgrid_size, L = pl->prm.grid_size;
-  const size_t nvis = (size_t)pl->B * pl->T * pl->C;
-  cudaStream_t s = S(stream);
-  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_uvw_dev, uvw_host, sizeof(float) * 3 * (size_t)pl->B * pl->T, cudaMemcpyHostToDevice, s));
-  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_vis_dev, vis_host, sizeof(float2) * 4 * nvis, cudaMemcpyHostToDevice, s));
-  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_aterms_dev, aterms_host, sizeof(float2) * 4 * N * N * (size_t)pl->n_stations * n_slots, cudaMemcpyHostToDevice, s));
-  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_taper_dev, taper_host, sizeof(float) * N * N, cudaMemcpyHostToDevice, s));
-  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_grid_dev, grid_host, sizeof(float2) * 4 * L * L, cudaMemcpyHostToDevice, s));
-  rc = idg_grid(pl, pl->h_uvw_dev, pl->h_vis_dev, pl->h_aterms_dev, pl->h_taper_dev, pl->h_grid_dev, stream);
+  const size_t row = (size_t)pl->T * pl->C * 4;                 // complex64 per baseline
+  cudaStream_t s = S(stream), c = pl->h_copy_stream;
+  const auto chunks = host_chunks(pl);
+  const int K = idg_plan::kHostChunks;
+  // the copy stream starts after whatever the caller queued on `stream`
+  IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_out[K], s));
+  IDG_CUDA_TRY(cudaStreamWaitEvent(c, pl->h_ev_out[K], 0));
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_uvw_dev, uvw_host, sizeof(float) * 3 * (size_t)pl->B * pl->T, cudaMemcpyHostToDevice, c));
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_aterms_dev, aterms_host, sizeof(float2) * 4 * N * N * (size_t)pl->n_stations * n_slots, cudaMemcpyHostToDevice, c));
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_taper_dev, taper_host, sizeof(float) * N * N, cudaMemcpyHostToDevice, c));
+  IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_in[K], c));
+  for (size_t k = 0; k < chunks.size(); ++k) {
+    const HostChunk &ch = chunks[k];
+    IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_vis_dev + (size_t)ch.b0 * row, (const float2 *)vis_host + (size_t)ch.b0 * row,
+                                 sizeof(float2) * row * (size_t)(ch.b1 - ch.b0), cudaMemcpyHostToDevice, c));
+    IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_in[k], c));
+  }
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_grid_dev, grid_host, sizeof(float2) * 4 * L * L, cudaMemcpyHostToDevice, c));
+  IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_in[K + 1], c));
+
+  IDG_CUDA_TRY(cudaStreamWaitEvent(s, pl->h_ev_in[K], 0));
+  for (size_t k = 0; k < chunks.size(); ++k) {
+    const HostChunk &ch = chunks[k];
+    IDG_CUDA_TRY(cudaStreamWaitEvent(s, pl->h_ev_in[k], 0));
+    rc = launch_gridder(pl, pl->h_uvw_dev, pl->h_vis_dev, pl->h_aterms_dev, pl->h_taper_dev, pl->subgrids_dev, s,
+                        ch.p0, ch.p1 - ch.p0);
+    if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, -1, s, ch.p0, ch.p1 - ch.p0);
+    if (rc != IDG_OK) return rc;
+  }
+  IDG_CUDA_TRY(cudaStreamWaitEvent(s, pl->h_ev_in[K + 1], 0));
+  rc = launch_adder(pl, pl->subgrids_dev, pl->h_grid_dev, s);
   if (rc != IDG_OK) return rc;
   IDG_CUDA_TRY(cudaMemcpyAsync(grid_host, pl->h_grid_dev, sizeof(float2) * 4 * L * L, cudaMemcpyDeviceToHost, s));
   IDG_CUDA_TRY(cudaStreamSynchronize(s));
@@ -128,20 +185,35 @@ int idg_degrid_host(idg_plan *pl, const float *uvw_host, const void *grid_host,
   if (!pl || !uvw_host || !vis_out_host || !aterms_host || !taper_host || !grid_host) return IDG_ERR_INVALID_ARG;
   if (n_slots < needed_slots(pl)) return IDG_ERR_PLAN_MISMATCH;
   int rc = ensure_staging(pl, n_slots);
+  if (rc == IDG_OK) rc = ensure_host_pipeline(pl);
   if (rc != IDG_OK) return rc;
   const size_t N = pl->prm.subgrid_size, L = pl->prm.grid_size;
+  const size_t row = (size_t)pl->T * pl->C * 4;
   const size_t nvis = (size_t)pl->B * pl->T * pl->C;
-  cudaStream_t s = S(stream);
+  cudaStream_t s = S(stream), c = pl->h_copy_stream;
+  const auto chunks = host_chunks(pl);
+  const int K = idg_plan::kHostChunks;
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_uvw_dev, uvw_host, sizeof(float) * 3 * (size_t)pl->B * pl->T, cudaMemcpyHostToDevice, s));
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_aterms_dev, aterms_host, sizeof(float2) * 4 * N * N * (size_t)pl->n_stations * n_slots, cudaMemcpyHostToDevice, s));
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_taper_dev, taper_host, sizeof(float) * N * N, cudaMemcpyHostToDevice, s));
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_grid_dev, grid_host, sizeof(float2) * 4 * L * L, cudaMemcpyHostToDevice, s));
-  if (pl->n_skipped == 0 && pl->P == 0)
+  if (pl->n_skipped > 0)   // skipped samples read as 0; planned ones are overwritten below
     IDG_CUDA_TRY(cudaMemsetAsync(pl->h_vis_dev, 0, sizeof(float2) * 4 * nvis, s));
-  rc = idg_degrid(pl, pl->h_uvw_dev, pl->h_grid_dev, pl->h_aterms_dev, pl->h_taper_dev, pl->h_vis_dev, stream);
-  if (rc != IDG_OK) return rc;
-  IDG_CUDA_TRY(cudaMemcpyAsync(vis_out_host, pl->h_vis_dev, sizeof(float2) * 4 * nvis, cudaMemcpyDeviceToHost, s));
+  for (size_t k = 0; k < chunks.size(); ++k) {
+    const HostChunk &ch = chunks[k];
+    rc = launch_splitter(pl, pl->h_grid_dev, pl->subgrids_dev, s, ch.p0, ch.p1 - ch.p0);
+    if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, +1, s, ch.p0, ch.p1 - ch.p0);
+    if (rc == IDG_OK)
+      rc = launch_degridder(pl, pl->h_uvw_dev, pl->subgrids_dev, pl->h_aterms_dev, pl->h_taper_dev, pl->h_vis_dev, s,
+                            ch.p0, ch.p1 - ch.p0);
+    if (rc != IDG_OK) return rc;
+    IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_out[k], s));
+    IDG_CUDA_TRY(cudaStreamWaitEvent(c, pl->h_ev_out[k], 0));
+    IDG_CUDA_TRY(cudaMemcpyAsync((float2 *)vis_out_host + (size_t)ch.b0 * row, pl->h_vis_dev + (size_t)ch.b0 * row,
+                                 sizeof(float2) * row * (size_t)(ch.b1 - ch.b0), cudaMemcpyDeviceToHost, c));
+  }
   IDG_CUDA_TRY(cudaStreamSynchronize(s));
+  IDG_CUDA_TRY(cudaStreamSynchronize(c));
   return IDG_OK;
 }
 

@@ -41,6 +41,11 @@ struct idg_plan {
   float2 *h_vis_dev = nullptr, *h_aterms_dev = nullptr, *h_grid_dev = nullptr;
   float *h_taper_dev = nullptr;
   int64_t h_aterm_slots = 0;
+  // copy/compute overlap of the *_host entry points: a copy stream and per-chunk events (created on first use)
+  cudaStream_t h_copy_stream = nullptr;
+  static constexpr int kHostChunks = 8;
+  cudaEvent_t h_ev_in[kHostChunks + 2] = {};    // chunk uploads, then [kHostChunks] = small inputs, [+1] = grid
+  cudaEvent_t h_ev_out[kHostChunks + 1] = {};   // chunk results ready on the compute stream, [kHostChunks] = start
 };
 
 namespace idg {
@@ -63,15 +68,18 @@ int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *
                 int64_t *planned, int64_t *skipped, cudaStream_t stream);
 
 // stage launchers (one .cu each); all asynchronous on `stream`
+// p0 / np select the subgrids [p0, p0 + np) of the plan (np < 0: all); `subgrids` is always the base of the
+// full [P][4][N][N] array.  The host-buffer entry points use ranges to overlap copies with compute.
 int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
-                   const float *taper, float2 *subgrids, cudaStream_t stream);
+                   const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0 = 0, int64_t np = -1);
 int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgrids,
                      const float2 *aterms, const float *taper, float2 *vis_out,
-                     cudaStream_t stream);
-int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream);
+                     cudaStream_t stream, int64_t p0 = 0, int64_t np = -1);
+int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream,
+                       int64_t p0 = 0, int64_t np = -1);
 int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cudaStream_t stream);
 int launch_splitter(const idg_plan *plan, const float2 *grid, float2 *subgrids,
-                    cudaStream_t stream);
+                    cudaStream_t stream, int64_t p0 = 0, int64_t np = -1);
 
 // packed FP32 FMA (sm_100 FFMA2): d = a * b + c on both halves
 __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {

@@ -140,9 +140,11 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
 
 template <int N, int NT, int CPT>
 static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgrids,
-                    const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream) {
-  degridder_kernel<N, NT, CPT><<<(unsigned)plan->P, NT, 0, stream>>>(
-      plan->meta_dev, uvw, plan->freqs_dev, subgrids, reinterpret_cast<const float4 *>(aterms),
+                    const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
+                    int64_t p0, int64_t np) {
+  degridder_kernel<N, NT, CPT><<<(unsigned)np, NT, 0, stream>>>(
+      plan->meta_dev + p0, uvw, plan->freqs_dev, subgrids + (size_t)p0 * 4 * N * N,
+      reinterpret_cast<const float4 *>(aterms),
       taper, reinterpret_cast<float4 *>(vis_out), plan->T, plan->C, plan->n_stations,
       plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
   IDG_CUDA_TRY(cudaGetLastError());
@@ -151,7 +153,8 @@ static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgri
 
 template <int N>
 static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgrids,
-                    const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream) {
+                    const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
+                    int64_t p0, int64_t np) {
   // threads own (timestep, CPT channels); pick CPT and the CTA size from the plan's largest block
   const int mc = plan->max_n_chan;
   // more channels per thread amortise the per-pixel shared-memory reads and phase set-up, as long as the
@@ -161,8 +164,8 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
   const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
   const bool small = items <= 128;
 #define IDG_DG(CPT_)                                                                         \
-  return small ? launch_k<N, 128, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream) \
-               : launch_k<N, 256, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream)
+  return small ? launch_k<N, 128, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np) \
+               : launch_k<N, 256, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np)
   if (cpt == 8) { IDG_DG(8); }
   if (cpt == 4) { IDG_DG(4); }
   if (cpt == 2) { IDG_DG(2); }
@@ -172,13 +175,14 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
 
 int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgrids,
                      const float2 *aterms, const float *taper, float2 *vis_out,
-                     cudaStream_t stream) {
-  if (plan->P == 0) return IDG_OK;
+                     cudaStream_t stream, int64_t p0, int64_t np) {
+  if (np < 0) np = plan->P - p0;
+  if (np <= 0) return IDG_OK;
   switch (plan->prm.subgrid_size) {
-    case 16: return launch_n<16>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
-    case 24: return launch_n<24>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
-    case 32: return launch_n<32>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
-    case 48: return launch_n<48>(plan, uvw, subgrids, aterms, taper, vis_out, stream);
+    case 16: return launch_n<16>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    case 24: return launch_n<24>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    case 32: return launch_n<32>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    case 48: return launch_n<48>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 }

@@ -168,26 +168,27 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
 
 template <int N, int NT, int PPT, int MINB>
 static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
-                    const float *taper, float2 *subgrids, cudaStream_t stream) {
+                    const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
   constexpr size_t smem = sizeof(float4) * (kVisBatch * 4 + N * N) + sizeof(float) * kMaxChan;
   auto kern = gridder_kernel<N, NT, PPT, MINB>;
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  kern<<<(unsigned)plan->P, NT, smem, stream>>>(
-      plan->meta_dev, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
-      reinterpret_cast<const float4 *>(aterms), taper, subgrids, plan->T, plan->C,
+  kern<<<(unsigned)np, NT, smem, stream>>>(
+      plan->meta_dev + p0, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
+      reinterpret_cast<const float4 *>(aterms), taper, subgrids + (size_t)p0 * 4 * N * N, plan->T, plan->C,
       plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
   IDG_CUDA_TRY(cudaGetLastError());
   return IDG_OK;
 }
 
 int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
-                   const float *taper, float2 *subgrids, cudaStream_t stream) {
-  if (plan->P == 0) return IDG_OK;
+                   const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
+  if (np < 0) np = plan->P - p0;
+  if (np <= 0) return IDG_OK;
   switch (plan->prm.subgrid_size) {
-    case 16: return launch_n<16, 64, 4, 8>(plan, uvw, vis, aterms, taper, subgrids, stream);
-    case 24: return launch_n<24, 96, 6, 5>(plan, uvw, vis, aterms, taper, subgrids, stream);
-    case 32: return launch_n<32, 256, 4, 2>(plan, uvw, vis, aterms, taper, subgrids, stream);
-    case 48: return launch_n<48, 384, 6, 1>(plan, uvw, vis, aterms, taper, subgrids, stream);
+    case 16: return launch_n<16, 64, 4, 8>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 24: return launch_n<24, 96, 6, 5>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 32: return launch_n<32, 256, 4, 2>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 48: return launch_n<48, 384, 6, 1>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 }

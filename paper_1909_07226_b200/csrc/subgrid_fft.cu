@@ -68,28 +68,32 @@ subgrid_fft_kernel(float2 *__restrict__ subgrids) {
 }
 
 template <int N>
-static int launch_n(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream) {
+static int launch_n(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream, int64_t p0,
+                    int64_t np) {
+  subgrids += (size_t)p0 * 4 * N * N;
   constexpr size_t smem = sizeof(float2) * 4 * N * (N + 1);
   if (direction < 0) {
     IDG_CUDA_TRY(cudaFuncSetAttribute(subgrid_fft_kernel<N, false>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    subgrid_fft_kernel<N, false><<<(unsigned)plan->P, 4 * N, smem, stream>>>(subgrids);
+    subgrid_fft_kernel<N, false><<<(unsigned)np, 4 * N, smem, stream>>>(subgrids);
   } else {
     IDG_CUDA_TRY(cudaFuncSetAttribute(subgrid_fft_kernel<N, true>,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    subgrid_fft_kernel<N, true><<<(unsigned)plan->P, 4 * N, smem, stream>>>(subgrids);
+    subgrid_fft_kernel<N, true><<<(unsigned)np, 4 * N, smem, stream>>>(subgrids);
   }
   IDG_CUDA_TRY(cudaGetLastError());
   return IDG_OK;
 }
 
-int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream) {
-  if (plan->P == 0) return IDG_OK;
+int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream, int64_t p0,
+                       int64_t np) {
+  if (np < 0) np = plan->P - p0;
+  if (np <= 0) return IDG_OK;
   switch (plan->prm.subgrid_size) {
-    case 16: return launch_n<16>(plan, subgrids, direction, stream);
-    case 24: return launch_n<24>(plan, subgrids, direction, stream);
-    case 32: return launch_n<32>(plan, subgrids, direction, stream);
-    case 48: return launch_n<48>(plan, subgrids, direction, stream);
+    case 16: return launch_n<16>(plan, subgrids, direction, stream, p0, np);
+    case 24: return launch_n<24>(plan, subgrids, direction, stream, p0, np);
+    case 32: return launch_n<32>(plan, subgrids, direction, stream, p0, np);
+    case 48: return launch_n<48>(plan, subgrids, direction, stream, p0, np);
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 }
