@@ -159,6 +159,22 @@ int idg_image_w_apply(void *out_dev, const void *in_dev, int32_t L, double image
                       void *cuda_stream);
 int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *cuda_stream);
 
+/* ---- scalar variant: one polarisation ------------------------------------------
+ * The method as the paper derives it before the 2x2 substitution (Eq. 1-25);
+ * "Stokes I only" is how the classical gridder is timed in PAPER.md:481.  Complex gains g (Eq. 2):
+ *   gridding   Sg = taper conj(g1) (sum_k Y_k exp(+i phase)) g2 ;  degridding  Y_k = sum_xy g1 (taper Ip) conj(g2) exp(-i phase)
+ * = the XX plane of the 4-polarisation calls with Jones matrices g I_2.  Same plan object, same conventions.
+ *   vis / vis_out [B][T][C] complex64, gains [slots][stations][N][N] complex64, grid [L][L] complex64,
+ *   subgrids [P][N][N] complex64 (idg_grid_scalar / idg_degrid_scalar use the plan's scratch). */
+int idg_grid_scalar(const idg_plan *plan, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+                    const float *taper_dev, void *grid_dev, void *cuda_stream);
+int idg_degrid_scalar(const idg_plan *plan, const float *uvw_dev, const void *grid_dev, const void *gains_dev,
+                      const float *taper_dev, void *vis_out_dev, void *cuda_stream);
+int idg_gridder_scalar(const idg_plan *plan, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+                       const float *taper_dev, void *subgrids_dev, void *cuda_stream);
+int idg_degridder_scalar(const idg_plan *plan, const float *uvw_dev, const void *subgrids_dev, const void *gains_dev,
+                         const float *taper_dev, void *vis_out_dev, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

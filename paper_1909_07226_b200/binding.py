@@ -26,7 +26,7 @@ EXPORTS = (
     "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
     "idg_adder", "idg_splitter", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
-    "idg_image_divide")
+    "idg_image_divide", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
 
 
 class IdgError(RuntimeError):
@@ -320,3 +320,46 @@ def idg_image_divide(image, cbar, stream=None) -> None:
         raise IdgError("image must be [4][L][L] and cbar [L][L]")
     _check(lib().idg_image_divide(_dev(image, _C64, "image"), _dev(cbar, _F32, "cbar"), ctypes.c_int32(L),
                                   _stream(stream)), "idg_image_divide")
+
+
+def _scalar_check(plan: Plan, uvw, vis, gains, taper, grid=None, subgrids=None):
+    N, L = int(plan.params.subgrid_size), int(plan.params.grid_size)
+    if tuple(uvw.shape) != (plan.B, plan.T, 3) or tuple(vis.shape) != (plan.B, plan.T, plan.C):
+        raise IdgError("scalar variant: uvw must be [B][T][3] and vis [B][T][C]")
+    g = tuple(gains.shape)
+    if len(g) != 4 or g[1:] != (plan.n_stations, N, N) or g[0] < plan.slots_needed():
+        raise IdgError("scalar variant: gains must be [slots >= %d][%d][%d][%d]" % (plan.slots_needed(), plan.n_stations, N, N))
+    if tuple(taper.shape) != (N, N):
+        raise IdgError("taper shape")
+    if grid is not None and tuple(grid.shape) != (L, L):
+        raise IdgError("scalar variant: grid must be [L][L]")
+    if subgrids is not None and tuple(subgrids.shape) != (plan.size()[0], N, N):
+        raise IdgError("scalar variant: subgrids must be [P][N][N]")
+
+
+def idg_grid_scalar(plan: Plan, uvw, vis, gains, taper, grid, stream=None) -> None:
+    """Scalar (one polarisation) Alg. 1; accumulates into grid [L][L] (NEXT-3)."""
+    _scalar_check(plan, uvw, vis, gains, taper, grid=grid)
+    _check(lib().idg_grid_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"), _dev(gains, _C64, "gains"),
+                                 _dev(taper, _F32, "taper"), _dev(grid, _C64, "grid"), _stream(stream)), "idg_grid_scalar")
+
+
+def idg_degrid_scalar(plan: Plan, uvw, grid, gains, taper, vis_out, stream=None) -> None:
+    _scalar_check(plan, uvw, vis_out, gains, taper, grid=grid)
+    _check(lib().idg_degrid_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(grid, _C64, "grid"), _dev(gains, _C64, "gains"),
+                                   _dev(taper, _F32, "taper"), _dev(vis_out, _C64, "vis_out"), _stream(stream)),
+           "idg_degrid_scalar")
+
+
+def idg_gridder_scalar(plan: Plan, uvw, vis, gains, taper, subgrids, stream=None) -> None:
+    _scalar_check(plan, uvw, vis, gains, taper, subgrids=subgrids)
+    _check(lib().idg_gridder_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"), _dev(gains, _C64, "gains"),
+                                    _dev(taper, _F32, "taper"), _dev(subgrids, _C64, "subgrids"), _stream(stream)),
+           "idg_gridder_scalar")
+
+
+def idg_degridder_scalar(plan: Plan, uvw, subgrids, gains, taper, vis_out, stream=None) -> None:
+    _scalar_check(plan, uvw, vis_out, gains, taper, subgrids=subgrids)
+    _check(lib().idg_degridder_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(subgrids, _C64, "subgrids"),
+                                      _dev(gains, _C64, "gains"), _dev(taper, _F32, "taper"),
+                                      _dev(vis_out, _C64, "vis_out"), _stream(stream)), "idg_degridder_scalar")

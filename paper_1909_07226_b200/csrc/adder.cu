@@ -23,23 +23,23 @@ __device__ __forceinline__ void red_add_f32x2(float2 *addr, float2 v) {
   asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(v.x), "f"(v.y) : "memory");
 }
 
-template <int N>
+template <int N, int NPOL>
 __global__ void __launch_bounds__(256)
 adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
              const idg_subgrid_meta *__restrict__ meta, const float2 *__restrict__ subgrids,
              float2 *__restrict__ grid, int32_t L) {
-  // The tile accumulator lives in shared memory, [pol][row][x].  Warp w owns polarisation w & 3 and
-  // the rows (w >> 2) + 2k of the tile: every (pol, row) slot has exactly one writer, so the
+  // The tile accumulator lives in shared memory, [pol][row][x].  Warp w owns polarisation w % NPOL and
+  // the rows w / NPOL + (8 / NPOL) k of the tile: every (pol, row) slot has exactly one writer, so the
   // accumulation needs neither atomics nor barriers, and a warp always reads whole subgrid rows
   // (N consecutive float2: 256 B at N = 32), one lane per pixel.
-  constexpr int TX = kAdderTileX, TY = kAdderTileY, ROWS = TY / 2;
+  constexpr int TX = kAdderTileX, TY = kAdderTileY, RSTEP = 8 / NPOL, ROWS = TY / RSTEP;
   constexpr int PASSES = (N + 31) / 32;            // N = 48: a row takes two passes of 32 lanes
-  __shared__ float2 tile[4][TY][TX];
+  __shared__ float2 tile[NPOL][TY][TX];
   const AdderItem it = items[blockIdx.x];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = warp & 3, r0 = warp >> 2;
+  const int q = warp % NPOL, r0 = warp / NPOL;
   const int xw = it.x_hi - it.x_lo;                // only the columns this item's subgrids cover
-  for (int i = threadIdx.x; i < 4 * TY * xw; i += 256) tile[i / (TY * xw)][(i / xw) % TY][it.x_lo + i % xw] = make_float2(0.f, 0.f);
+  for (int i = threadIdx.x; i < NPOL * TY * xw; i += 256) tile[i / (TY * xw)][(i / xw) % TY][it.x_lo + i % xw] = make_float2(0.f, 0.f);
   __syncthreads();
 
   for (int e0 = it.begin; e0 < it.end; e0 += 2) {   // two subgrids per trip: twice the loads in flight
@@ -52,10 +52,10 @@ adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
       const int4 ent = have ? __ldg(&list[e0 + j]) : make_int4(0, 0, 0, 0);
       tx0[j] = ent.y;
       const int sy0 = r0 - ent.z;
-      const float2 *sg = subgrids + ((size_t)ent.x * 4 + q) * N * N;
+      const float2 *sg = subgrids + ((size_t)ent.x * NPOL + q) * N * N;
 #pragma unroll
       for (int k = 0; k < ROWS; ++k) {
-        const int sy = sy0 + 2 * k;
+        const int sy = sy0 + RSTEP * k;
         ok[j][k] = have && sy >= 0 && sy < N;
 #pragma unroll
         for (int p = 0; p < PASSES; ++p) {
@@ -73,16 +73,16 @@ adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
           for (int p = 0; p < PASSES; ++p) {
             const int sx = lane + 32 * p, x = tx0[j] + sx;
             if (sx < N && x >= 0 && x < TX) {
-              float2 a = tile[q][r0 + 2 * k][x];
+              float2 a = tile[q][r0 + RSTEP * k][x];
               a.x += v[j][k][p].x; a.y += v[j][k][p].y;
-              tile[q][r0 + 2 * k][x] = a;
+              tile[q][r0 + RSTEP * k][x] = a;
             }
           }
         }
   }
   __syncthreads();
   // one vector reduction per touched pixel of the tile (untouched ones hold exact zeros and are skipped)
-  for (int i = threadIdx.x; i < 4 * TY * xw; i += 256) {
+  for (int i = threadIdx.x; i < NPOL * TY * xw; i += 256) {
     const int x = it.x_lo + i % xw, r = (i / xw) % TY, qq = i / (TY * xw);
     const float2 a = tile[qq][r][x];
     const int gx = it.tile_x + x, gy = it.tile_y + r;
@@ -90,25 +90,27 @@ adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
   }
 }
 
-template <int N>
+template <int N, int NPOL>
 __global__ void __launch_bounds__(256)
 splitter_kernel(const idg_subgrid_meta *__restrict__ meta, const float2 *__restrict__ grid,
                 float2 *__restrict__ subgrids, int32_t L) {
   const int x0 = meta[blockIdx.x].x0, y0 = meta[blockIdx.x].y0;
-  float2 *sg = subgrids + (size_t)blockIdx.x * 4 * N * N;
+  float2 *sg = subgrids + (size_t)blockIdx.x * NPOL * N * N;
 #pragma unroll 4
-  for (int e = threadIdx.x; e < 4 * N * N; e += 256) {
+  for (int e = threadIdx.x; e < NPOL * N * N; e += 256) {
     const int q = e / (N * N), r = e - q * N * N;
     const int y = r / N, x = r - y * N;
     sg[e] = __ldg(&grid[((size_t)q * L + (y0 + y)) * L + (x0 + x)]);
   }
 }
 
-int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cudaStream_t stream) {
+int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cudaStream_t stream, int n_pol) {
   if (plan->n_adder_items == 0) return IDG_OK;
   const unsigned nb = (unsigned)plan->n_adder_items;
   const int32_t L = plan->prm.grid_size;
-#define IDG_ADD(N_) adder_kernel<N_><<<nb, 256, 0, stream>>>(plan->adder_items_dev, plan->adder_list_dev, plan->meta_dev, subgrids, grid, L)
+#define IDG_ADD(N_)                                                                                          \
+  if (n_pol == 1) adder_kernel<N_, 1><<<nb, 256, 0, stream>>>(plan->adder_items_dev, plan->adder_list_dev, plan->meta_dev, subgrids, grid, L); \
+  else adder_kernel<N_, 4><<<nb, 256, 0, stream>>>(plan->adder_items_dev, plan->adder_list_dev, plan->meta_dev, subgrids, grid, L)
   switch (plan->prm.subgrid_size) {
     case 16: IDG_ADD(16); break;
     case 24: IDG_ADD(24); break;
@@ -122,13 +124,15 @@ int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cud
 }
 
 int launch_splitter(const idg_plan *plan, const float2 *grid, float2 *subgrids,
-                    cudaStream_t stream, int64_t p0, int64_t np) {
+                    cudaStream_t stream, int64_t p0, int64_t np, int n_pol) {
   if (np < 0) np = plan->P - p0;
   if (np <= 0) return IDG_OK;
   const unsigned nb = (unsigned)np;
-  subgrids += (size_t)p0 * 4 * plan->prm.subgrid_size * plan->prm.subgrid_size;
+  subgrids += (size_t)p0 * n_pol * plan->prm.subgrid_size * plan->prm.subgrid_size;
   const int32_t L = plan->prm.grid_size;
-#define IDG_SPL(N_) splitter_kernel<N_><<<nb, 256, 0, stream>>>(plan->meta_dev + p0, grid, subgrids, L)
+#define IDG_SPL(N_)                                                                          \
+  if (n_pol == 1) splitter_kernel<N_, 1><<<nb, 256, 0, stream>>>(plan->meta_dev + p0, grid, subgrids, L); \
+  else splitter_kernel<N_, 4><<<nb, 256, 0, stream>>>(plan->meta_dev + p0, grid, subgrids, L)
   switch (plan->prm.subgrid_size) {
     case 16: IDG_SPL(16); break;
     case 24: IDG_SPL(24); break;

@@ -103,6 +103,45 @@ int idg_degrid(const idg_plan *pl, const float *uvw_dev, const void *grid_dev,
   return rc;
 }
 
+// ---- scalar variant (NEXT-3): one polarisation; subgrids [P][N][N] live in the first quarter of the plan's
+// scratch; the plane-wise FFT kernel sees them as ceil(P / 4) four-plane subgrids ------------------------------
+int idg_gridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+                       const float *taper_dev, void *subgrids_dev, void *stream) {
+  if (!pl || !uvw_dev || !vis_dev || !gains_dev || !taper_dev || (!subgrids_dev && pl->P > 0)) return IDG_ERR_INVALID_ARG;
+  return launch_gridder_scalar(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)gains_dev, taper_dev,
+                               (float2 *)subgrids_dev, S(stream));
+}
+
+int idg_degridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *subgrids_dev, const void *gains_dev,
+                         const float *taper_dev, void *vis_out_dev, void *stream) {
+  if (!pl || !uvw_dev || (!subgrids_dev && pl->P > 0) || !gains_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
+  return launch_degridder_scalar(pl, uvw_dev, (const float2 *)subgrids_dev, (const float2 *)gains_dev, taper_dev,
+                                 (float2 *)vis_out_dev, S(stream));
+}
+
+int idg_grid_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+                    const float *taper_dev, void *grid_dev, void *stream) {
+  if (!pl || !uvw_dev || !vis_dev || !gains_dev || !taper_dev || !grid_dev) return IDG_ERR_INVALID_ARG;
+  int rc = launch_gridder_scalar(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)gains_dev, taper_dev,
+                                 pl->subgrids_dev, S(stream));
+  if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, -1, S(stream), 0, (pl->P + 3) / 4);
+  if (rc == IDG_OK) rc = launch_adder(pl, pl->subgrids_dev, (float2 *)grid_dev, S(stream), 1);
+  return rc;
+}
+
+int idg_degrid_scalar(const idg_plan *pl, const float *uvw_dev, const void *grid_dev, const void *gains_dev,
+                      const float *taper_dev, void *vis_out_dev, void *stream) {
+  if (!pl || !uvw_dev || !grid_dev || !gains_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
+  if (pl->n_skipped > 0)
+    IDG_CUDA_TRY(cudaMemsetAsync(vis_out_dev, 0, sizeof(float2) * (size_t)pl->B * pl->T * pl->C, S(stream)));
+  int rc = launch_splitter(pl, (const float2 *)grid_dev, pl->subgrids_dev, S(stream), 0, -1, 1);
+  if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, +1, S(stream), 0, (pl->P + 3) / 4);
+  if (rc == IDG_OK)
+    rc = launch_degridder_scalar(pl, uvw_dev, pl->subgrids_dev, (const float2 *)gains_dev, taper_dev,
+                                 (float2 *)vis_out_dev, S(stream));
+  return rc;
+}
+
 // The host-buffer calls overlap the PCIe copies with the kernels: the baselines are cut into kHostChunks
 // contiguous ranges (the metadata is sorted by baseline, so a range of baselines is a range of subgrids and a
 // contiguous slice of vis); uploads run on the plan's copy stream, kernels on the caller's stream, events

@@ -77,9 +77,14 @@ int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgr
                      cudaStream_t stream, int64_t p0 = 0, int64_t np = -1);
 int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream,
                        int64_t p0 = 0, int64_t np = -1);
-int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cudaStream_t stream);
+int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cudaStream_t stream, int n_pol = 4);
 int launch_splitter(const idg_plan *plan, const float2 *grid, float2 *subgrids,
-                    cudaStream_t stream, int64_t p0 = 0, int64_t np = -1);
+                    cudaStream_t stream, int64_t p0 = 0, int64_t np = -1, int n_pol = 4);
+// scalar variant (NEXT-3, scalar.cu): vis [B][T][C], gains [slots][stations][N][N], subgrids [P][N][N]
+int launch_gridder_scalar(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *gains,
+                          const float *taper, float2 *subgrids, cudaStream_t stream);
+int launch_degridder_scalar(const idg_plan *plan, const float *uvw, const float2 *subgrids, const float2 *gains,
+                            const float *taper, float2 *vis_out, cudaStream_t stream);
 
 // packed FP32 FMA (sm_100 FFMA2): d = a * b + c on both halves
 __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {

@@ -442,3 +442,59 @@ def test_w_stacked_dirty_image_and_prediction():
     got = imaging.predict(prm, wc.uvw, w.freqs, w.baselines, w.n_stations, torch.from_numpy(model).cuda(),
                           wc.aterms, wc.taper, w.C)
     assert H.rel_l2(got.cpu().numpy(), ref_vis) < TOL
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3: scalar (one polarisation) variant = XX plane of the 4-polarisation oracle with Jones matrices g I_2
+# ---------------------------------------------------------------------------------------------
+
+def _scalar_inputs(w, rng):
+    """Scalar visibilities and gains, and the 4-polarisation arrays that embed them."""
+    N = w.params.subgrid_size
+    vis_s = w.vis.numpy()[..., 0].copy()                                   # [B][T][C]
+    n_slots = w.aterms.shape[0]
+    g = (1.0 + 0.1 * (rng.standard_normal((n_slots, w.n_stations, N, N)) +
+                      1j * rng.standard_normal((n_slots, w.n_stations, N, N)))).astype(np.complex64)
+    vis4 = np.zeros(w.vis.shape, dtype=np.complex64)
+    vis4[..., 0] = vis_s
+    at4 = np.zeros((n_slots, w.n_stations, N, N, 4), dtype=np.complex64)
+    at4[..., 0] = g
+    at4[..., 3] = g
+    return vis_s, g, vis4, at4
+
+
+@pytest.mark.parametrize("name,kw", [("tiny", {}), ("lofar", dict(n_baselines=40, baseline_offset=600, n_time=128))])
+def test_scalar_variant_matches_xx_plane_of_the_oracle(name, kw):
+    w = synth.make_workload(name, **kw)
+    prm = dataclasses.replace(w.params, w_step=150.0) if name == "tiny" else w.params
+    rng = np.random.default_rng(17)
+    vis_s, g, vis4, at4 = _scalar_inputs(w, rng)
+    uvw, taper = w.uvw.numpy(), w.taper.numpy()
+    d_uvw = w.uvw.cuda()
+    plan = idg.idg_plan_create(prm, d_uvw, w.freqs, w.baselines, w.n_stations)
+    meta, _, _ = orc.plan(prm, uvw, w.freqs, w.baselines)
+    assert plan.metadata().tobytes() == meta.tobytes()
+    L, N, P = prm.grid_size, prm.subgrid_size, len(meta)
+    d_vis, d_g, d_tp = torch.from_numpy(vis_s).cuda(), torch.from_numpy(g).cuda(), w.taper.cuda()
+    # stage: gridder
+    ref_img = orc.gridder(prm, meta, uvw, w.freqs, vis4, at4, taper)[:, 0]
+    sub = torch.zeros((P, N, N), dtype=torch.complex64, device="cuda")
+    idg.idg_gridder_scalar(plan, d_uvw, d_vis, d_g, d_tp, sub)
+    torch.cuda.synchronize()
+    got = sub.cpu().numpy()
+    assert max(H.rel_l2(got[p], ref_img[p]) for p in range(P)) < TOL
+    # Alg. 1
+    ref_grid = orc.grid(prm, meta, uvw, w.freqs, vis4, at4, taper)[0]
+    grid = torch.zeros((L, L), dtype=torch.complex64, device="cuda")
+    idg.idg_grid_scalar(plan, d_uvw, d_vis, d_g, d_tp, grid)
+    torch.cuda.synchronize()
+    assert H.rel_l2(grid.cpu().numpy(), ref_grid) < TOL
+    # Alg. 2 on a random model grid (XX plane only: the other planes of the embedding are zero)
+    model = (rng.standard_normal((L, L)) + 1j * rng.standard_normal((L, L))).astype(np.complex64)
+    model4 = np.zeros((4, L, L), dtype=np.complex128)
+    model4[0] = model
+    ref_vis = orc.degrid(prm, meta, uvw, w.freqs, model4, at4, taper, w.B)[..., 0]
+    out = torch.full(d_vis.shape, 5.0, dtype=torch.complex64, device="cuda")
+    idg.idg_degrid_scalar(plan, d_uvw, torch.from_numpy(model).cuda(), d_g, d_tp, out)
+    torch.cuda.synchronize()
+    assert H.rel_l2(out.cpu().numpy(), ref_vis) < TOL
