@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/idg_b200.h: argument checks, plan ownership, stage sequencing.
 #include <algorithm>
+#include <cmath>
 #include <cstring>
 #include <new>
 
@@ -91,6 +92,14 @@ static int finish_plan(idg_plan *pl, const double *freqs_host, cudaStream_t stre
   for (const auto &m : pl->meta_host) {
     pl->max_n_time = std::max(pl->max_n_time, m.n_time);
     pl->max_n_chan = std::max(pl->max_n_chan, m.n_chan);
+  }
+  pl->uniform_dkd = 0.f;
+  if (pl->C >= 2) {
+    const double df = freqs_host[1] - freqs_host[0];
+    bool uniform = df != 0.0;
+    for (int32_t c = 1; c + 1 < pl->C; ++c)
+      uniform = uniform && std::fabs((freqs_host[c + 1] - freqs_host[c]) - df) <= 1e-9 * std::fabs(df);
+    if (uniform) pl->uniform_dkd = (float)(6.283185307179586476925286766559 * df / kSpeedOfLight);
   }
   IDG_CUDA_TRY(cudaMalloc(&pl->freqs_dev, sizeof(double) * pl->C));
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->freqs_dev, freqs_host, sizeof(double) * pl->C,

@@ -17,13 +17,13 @@ namespace idg {
 constexpr int kSVisBatch = 512;   // scalar visibilities staged per batch (8 B each)
 constexpr int kSMaxChan = 256;
 
-template <int N, int NT, int PPT, int MINB>
+template <int N, int NT, int PPT, int MINB, int R>
 __global__ void __launch_bounds__(NT, MINB)
 gridder_scalar_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                       const double *__restrict__ freqs, const float2 *__restrict__ vis,
                       const float2 *__restrict__ gains, const float *__restrict__ taper,
                       float2 *__restrict__ subgrids, int32_t T, int32_t C, int32_t n_stations, int32_t L,
-                      double image_size, double w_step) {
+                      double image_size, double w_step, float dkd) {
   static_assert(NT * PPT == N * N, "pixels must tile the CTA exactly");
   __shared__ float2 s_vis[kSVisBatch];
   __shared__ float4 s_t[kSVisBatch * 2];
@@ -82,16 +82,46 @@ gridder_scalar_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__
           base[k] = fmaf(tbs.x, pl[k], fmaf(tbs.y, pm[k], tbs.z * pn[k]));
         }
         const float2 *vp = s_vis + (size_t)tl * nc;
+        if (R == 1) {
 #pragma unroll 4
-        for (int c = 0; c < nc; ++c) {
-          const float kd = s_kd[c_lo + c];
-          const float2 v = vp[c];
+          for (int c = 0; c < nc; ++c) {
+            const float kd = s_kd[c_lo + c];
+            const float2 v = vp[c];
 #pragma unroll
-          for (int k = 0; k < PPT; ++k) {
-            float s, co;
-            __sincosf(fmaf(pidx[k], kd, base[k]), &s, &co);
-            acc[k].x = fmaf(v.x, co, acc[k].x); acc[k].x = fmaf(-v.y, s, acc[k].x);
-            acc[k].y = fmaf(v.x, s, acc[k].y);  acc[k].y = fmaf(v.y, co, acc[k].y);
+            for (int k = 0; k < PPT; ++k) {
+              float s, co;
+              __sincosf(fmaf(pidx[k], kd, base[k]), &s, &co);
+              acc[k].x = fmaf(v.x, co, acc[k].x); acc[k].x = fmaf(-v.y, s, acc[k].x);
+              acc[k].y = fmaf(v.x, s, acc[k].y);  acc[k].y = fmaf(v.y, co, acc[k].y);
+            }
+          }
+        } else {
+          // per-channel phase recurrence (uniform channel spacing): sin/cos on every R-th channel, one complex
+          // rotation by exp(i pidx dkd) for the channels in between -- trades MUFU for FP32 FMAs
+          float cr[PPT], sr[PPT];
+#pragma unroll
+          for (int k = 0; k < PPT; ++k) __sincosf(pidx[k] * dkd, &sr[k], &cr[k]);
+          for (int c0 = 0; c0 < nc; c0 += R) {
+            const float kd = s_kd[c_lo + c0];
+            float co[PPT], sn[PPT];
+#pragma unroll
+            for (int k = 0; k < PPT; ++k) __sincosf(fmaf(pidx[k], kd, base[k]), &sn[k], &co[k]);
+#pragma unroll
+            for (int j = 0; j < R; ++j) {
+              if (c0 + j < nc) {
+                const float2 v = vp[c0 + j];
+#pragma unroll
+                for (int k = 0; k < PPT; ++k) {
+                  acc[k].x = fmaf(v.x, co[k], acc[k].x); acc[k].x = fmaf(-v.y, sn[k], acc[k].x);
+                  acc[k].y = fmaf(v.x, sn[k], acc[k].y); acc[k].y = fmaf(v.y, co[k], acc[k].y);
+                  if (j + 1 < R) {
+                    const float c2 = fmaf(co[k], cr[k], -sn[k] * sr[k]);
+                    sn[k] = fmaf(sn[k], cr[k], co[k] * sr[k]);
+                    co[k] = c2;
+                  }
+                }
+              }
+            }
           }
         }
       }
@@ -110,13 +140,13 @@ gridder_scalar_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__
   }
 }
 
-template <int N, int NT, int CPT>
+template <int N, int NT, int CPT, int R>
 __global__ void __launch_bounds__(NT)
 degridder_scalar_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                         const double *__restrict__ freqs, const float2 *__restrict__ subgrids,
                         const float2 *__restrict__ gains, const float *__restrict__ taper,
                         float2 *__restrict__ vis_out, int32_t T, int32_t C, int32_t n_stations, int32_t L,
-                        double image_size, double w_step) {
+                        double image_size, double w_step, float dkd) {
   constexpr int NPIX = N * N;
   constexpr int CH = NPIX < 1024 ? NPIX : 1024;
   __shared__ float2 s_pix[CH];
@@ -176,12 +206,31 @@ degridder_scalar_kernel(const idg_subgrid_meta *__restrict__ meta, const float *
           const float2 q = s_pix[i];
           const float pidx = fmaf(u, c3.x, fmaf(v, c3.y, w * c3.z));
           const float base = fmaf(bu, c3.x, fmaf(bv, c3.y, bw * c3.z));
+          if (R == 1) {
 #pragma unroll
-          for (int c = 0; c < CPT; ++c) {
-            float s, co;
-            __sincosf(fmaf(pidx, kd[c], base), &s, &co);
-            acc[c].x = fmaf(q.x, co, acc[c].x); acc[c].x = fmaf(q.y, s, acc[c].x);
-            acc[c].y = fmaf(q.y, co, acc[c].y); acc[c].y = fmaf(-q.x, s, acc[c].y);
+            for (int c = 0; c < CPT; ++c) {
+              float s, co;
+              __sincosf(fmaf(pidx, kd[c], base), &s, &co);
+              acc[c].x = fmaf(q.x, co, acc[c].x); acc[c].x = fmaf(q.y, s, acc[c].x);
+              acc[c].y = fmaf(q.y, co, acc[c].y); acc[c].y = fmaf(-q.x, s, acc[c].y);
+            }
+          } else {
+            float sr, cr;
+            __sincosf(pidx * dkd, &sr, &cr);
+#pragma unroll
+            for (int c0 = 0; c0 < CPT; c0 += R) {
+              float s, co;
+              __sincosf(fmaf(pidx, kd[c0], base), &s, &co);
+#pragma unroll
+              for (int j = 0; j < R && c0 + j < CPT; ++j) {
+                const int c = c0 + j;
+                acc[c].x = fmaf(q.x, co, acc[c].x); acc[c].x = fmaf(q.y, s, acc[c].x);
+                acc[c].y = fmaf(q.y, co, acc[c].y); acc[c].y = fmaf(-q.x, s, acc[c].y);
+                const float c2 = fmaf(co, cr, -s * sr);
+                s = fmaf(s, cr, co * sr);
+                co = c2;
+              }
+            }
           }
         }
       }
@@ -195,12 +244,22 @@ degridder_scalar_kernel(const idg_subgrid_meta *__restrict__ meta, const float *
   }
 }
 
+// channel spacing 2 pi df / c0 if the plan's channels are equally spaced (then the recurrence is exact up to
+// rounding), else 0: the kernels then evaluate sin/cos for every channel
+static float uniform_dkd(const idg_plan *plan) { return plan->uniform_dkd; }
+
 template <int N, int NT, int PPT, int MINB>
 static int launch_gs(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *gains,
                      const float *taper, float2 *subgrids, cudaStream_t stream) {
-  gridder_scalar_kernel<N, NT, PPT, MINB><<<(unsigned)plan->P, NT, 0, stream>>>(
-      plan->meta_dev, uvw, plan->freqs_dev, vis, gains, taper, subgrids, plan->T, plan->C, plan->n_stations,
-      plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
+  const float dkd = uniform_dkd(plan);
+  if (dkd != 0.f && plan->max_n_chan >= 4)
+    gridder_scalar_kernel<N, NT, PPT, MINB, 4><<<(unsigned)plan->P, NT, 0, stream>>>(
+        plan->meta_dev, uvw, plan->freqs_dev, vis, gains, taper, subgrids, plan->T, plan->C, plan->n_stations,
+        plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, dkd);
+  else
+    gridder_scalar_kernel<N, NT, PPT, MINB, 1><<<(unsigned)plan->P, NT, 0, stream>>>(
+        plan->meta_dev, uvw, plan->freqs_dev, vis, gains, taper, subgrids, plan->T, plan->C, plan->n_stations,
+        plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, 0.f);
   IDG_CUDA_TRY(cudaGetLastError());
   return IDG_OK;
 }
@@ -222,11 +281,13 @@ static int launch_ds(const idg_plan *plan, const float *uvw, const float2 *subgr
                      const float *taper, float2 *vis_out, cudaStream_t stream) {
   const int mc = plan->max_n_chan;
   const int cpt = mc >= 8 ? 8 : (mc >= 4 ? 4 : (mc >= 2 ? 2 : 1));
-#define IDG_DS(CPT_)                                                                                      \
-  degridder_scalar_kernel<N, 128, CPT_><<<(unsigned)plan->P, 128, 0, stream>>>(                           \
+  const float dkd = uniform_dkd(plan);
+#define IDG_DS(CPT_, R_)                                                                                  \
+  degridder_scalar_kernel<N, 128, CPT_, R_><<<(unsigned)plan->P, 128, 0, stream>>>(                       \
       plan->meta_dev, uvw, plan->freqs_dev, subgrids, gains, taper, vis_out, plan->T, plan->C,            \
-      plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step)
-  if (cpt == 8) IDG_DS(8); else if (cpt == 4) IDG_DS(4); else if (cpt == 2) IDG_DS(2); else IDG_DS(1);
+      plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, dkd)
+  if (cpt == 8 && dkd != 0.f) IDG_DS(8, 4); else if (cpt == 4 && dkd != 0.f) IDG_DS(4, 4);
+  else if (cpt == 8) IDG_DS(8, 1); else if (cpt == 4) IDG_DS(4, 1); else if (cpt == 2) IDG_DS(2, 1); else IDG_DS(1, 1);
 #undef IDG_DS
   IDG_CUDA_TRY(cudaGetLastError());
   return IDG_OK;

@@ -57,9 +57,12 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--reps", type=int, default=3)
     ap.add_argument("--quick", action="store_true")
+    ap.add_argument("--scalar", action="store_true", help="time the scalar (one polarisation) variant instead")
     args = ap.parse_args()
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
+    if args.scalar:
+        return scalar_report(dev, args.reps)
     hbm = 6451.2
     try:
         root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -106,6 +109,40 @@ def main():
         sys.stdout.flush()
         plan.destroy()
         del sub, out, aterms
+
+
+def scalar_report(dev, reps):
+    """NEXT-3: the scalar variant on the LOFAR-like and a 2000-baseline SKA-like slice, against the XU (MUFU)
+    roofline 148 SMs x 16 lanes x 1.965 GHz / (2 N^2) visibilities/s and against the 4-polarisation kernels."""
+    print("# Scalar (one polarisation) variant, NEXT-3")
+    print()
+    print("Command: `python -m paper_1909_07226_b200.sweep --scalar --reps %d`.  XU roofline = 148 x 16 x 1.965e9 / (2 N^2) vis/s." % reps)
+    print()
+    print("| workload | N | visibilities | scalar gridder ms | MVis/s | frac of XU roofline | scalar degridder ms | MVis/s | frac | "
+          "4-pol gridder ms | 4-pol degridder ms |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|")
+    for name, kw in (("lofar", {}), ("ska", dict(n_baselines=2000, baseline_offset=3000))):
+        w = synth.make_workload(name, device=dev, **kw)
+        N = w.params.subgrid_size
+        plan = idg.idg_plan_create(w.params, w.uvw, w.freqs, w.baselines, w.n_stations)
+        P, planned, _ = plan.size()
+        vis_s = w.vis[..., 0].contiguous()
+        gains = w.aterms[..., 0].contiguous()
+        sub4 = plan.subgrids()
+        sub1 = torch.view_as_complex(torch.view_as_real(sub4).reshape(-1)[: P * N * N * 2].reshape(P, N, N, 2))
+        out1 = torch.empty_like(vis_s)
+        out4 = torch.empty_like(w.vis)
+        tg = _time(lambda: idg.idg_gridder_scalar(plan, w.uvw, vis_s, gains, w.taper, sub1), reps)
+        td = _time(lambda: idg.idg_degridder_scalar(plan, w.uvw, sub1, gains, w.taper, out1), reps)
+        tg4 = _time(lambda: idg.idg_gridder(plan, w.uvw, w.vis, w.aterms, w.taper, sub4), reps)
+        td4 = _time(lambda: idg.idg_degridder(plan, w.uvw, sub4, w.aterms, w.taper, out4), reps)
+        roof = N_SM * 16 * HZ / (2.0 * N * N)
+        print("| %s | %d | %d | %.3f | %.0f | %.3f | %.3f | %.0f | %.3f | %.3f | %.3f |" %
+              (name, N, planned, tg, planned / tg / 1e3, planned / (tg * 1e-3) / roof, td, planned / td / 1e3,
+               planned / (td * 1e-3) / roof, tg4, td4))
+        sys.stdout.flush()
+        del sub1, sub4
+        plan.destroy()
 
 
 if __name__ == "__main__":

@@ -463,9 +463,14 @@ def _scalar_inputs(w, rng):
     return vis_s, g, vis4, at4
 
 
-@pytest.mark.parametrize("name,kw", [("tiny", {}), ("lofar", dict(n_baselines=40, baseline_offset=600, n_time=128))])
-def test_scalar_variant_matches_xx_plane_of_the_oracle(name, kw):
+@pytest.mark.parametrize("name,kw,uneven", [("tiny", {}, False), ("tiny", {}, True),
+                                            ("lofar", dict(n_baselines=40, baseline_offset=600, n_time=128), False)])
+def test_scalar_variant_matches_xx_plane_of_the_oracle(name, kw, uneven):
+    """Equally spaced channels take the phase-recurrence kernels (sin/cos every 4th channel), unevenly spaced
+    ones the direct kernels."""
     w = synth.make_workload(name, **kw)
+    if uneven:
+        w.freqs = w.freqs + np.array([0.0, 30e3, -20e3, 50e3])[: len(w.freqs)]
     prm = dataclasses.replace(w.params, w_step=150.0) if name == "tiny" else w.params
     rng = np.random.default_rng(17)
     vis_s, g, vis4, at4 = _scalar_inputs(w, rng)
