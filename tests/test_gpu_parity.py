@@ -503,3 +503,12 @@ def test_scalar_variant_matches_xx_plane_of_the_oracle(name, kw, uneven):
     idg.idg_degrid_scalar(plan, d_uvw, torch.from_numpy(model).cuda(), d_g, d_tp, out)
     torch.cuda.synchronize()
     assert H.rel_l2(out.cpu().numpy(), ref_vis) < TOL
+
+
+def test_ska_full_size_sampled():
+    """BASELINE.json configs[2] and [3] at full size (8128 baselines, 133 M visibilities, 8192^2 grid, ~266 k
+    subgrids) in the launch configuration bench.py --workload ska times: plan bit-exact against the oracle planner,
+    24 sampled subgrids / blocks against the oracle in both directions, adder by conservation and sampled windows."""
+    w = synth.make_workload("ska", device="cuda")            # generated on the GPU (seconds), checked from a host copy
+    host = dataclasses.replace(w, uvw=w.uvw.cpu(), vis=w.vis.cpu(), aterms=w.aterms.cpu(), taper=w.taper.cpu())
+    assert _sampled_full_size_check(host, 24, 31) > 250000
