@@ -45,6 +45,9 @@ typedef enum {
 } idg_status;
 
 #define IDG_PLAN_FORCE_BLOCKS 1 /* flags: blocks end only on max_timesteps / A-term slot (sweep mode) */
+#define IDG_PLAN_SPAN_ATERMS 2  /* flags (NEXT-4): a block may span A-term slots; the slot of timestep t is
+                                   t / aterm_interval and c_pk varies inside the visibility loop (section 3.4,
+                                   PAPER.md:247; Alg. 1); meta.aterm_slot = slot of the first timestep */
 
 /* Partitioning parameters (section 3.2; readings R10-R12).  All explicit. */
 typedef struct {
@@ -54,7 +57,7 @@ typedef struct {
   int32_t max_timesteps;  /* per subgrid, >= 1 */
   int32_t max_channels;   /* per subgrid, power of two */
   int32_t aterm_interval; /* timesteps per A-term slot, >= 1 (R5: a block never spans two slots) */
-  int32_t flags;          /* IDG_PLAN_FORCE_BLOCKS or 0 */
+  int32_t flags;          /* IDG_PLAN_FORCE_BLOCKS | IDG_PLAN_SPAN_ATERMS or 0 */
   int32_t reserved;       /* must be 0 */
   double image_size;      /* S: direction-cosine extent of the image; grid cell = 1/S wavelengths */
   double w_step;          /* w-layer thickness in wavelengths; 0 -> w0 = 0 for every subgrid (R4) */

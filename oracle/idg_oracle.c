@@ -42,6 +42,7 @@
 
 #define ORACLE_C0 299792458.0
 #define ORACLE_FORCE_BLOCKS 1
+#define ORACLE_SPAN_ATERMS 2 /* NEXT-4: a block may span A-term slots; c_pk then varies inside the k-sum */
 static const double ORACLE_TWO_PI = 6.283185307179586476925286766559;
 
 /* Same binary layout as the boundary's structs (the layout is the contract, the
@@ -84,6 +85,7 @@ int64_t oracle_plan(const oracle_params *prm, const float *uvw /*[B][T][3]*/,
                     int64_t *n_planned_vis, int64_t *n_skipped_vis) {
   const int32_t N = prm->subgrid_size, L = prm->grid_size;
   const int force = (prm->flags & ORACLE_FORCE_BLOCKS) != 0;
+  const int span = (prm->flags & ORACLE_SPAN_ATERMS) != 0;
   const double budget = (double)(N - prm->kernel_size);
   double *scale = (double *)malloc(sizeof(double) * (size_t)C);
   for (int32_t c = 0; c < C; ++c) scale[c] = (freqs[c] * (1.0 / ORACLE_C0)) * prm->image_size;
@@ -115,7 +117,7 @@ int64_t oracle_plan(const oracle_params *prm, const float *uvw /*[B][T][3]*/,
         double umin = 0, umax = 0, vmin = 0, vmax = 0;
         int32_t wi0 = 0;
         while (t1 < T && t1 - t0 < prm->max_timesteps &&
-               t1 / prm->aterm_interval == t0 / prm->aterm_interval) {
+               (span || t1 / prm->aterm_interval == t0 / prm->aterm_interval)) {
           int32_t wi = 0;
           if (prm->w_step > 0.0)
             wi = (int32_t)floor(((double)uvw_b[3 * t1 + 2] * k_mid) / prm->w_step);
@@ -219,6 +221,35 @@ void oracle_gridder(const oracle_params *prm, const oracle_meta *meta, int64_t P
     for (int32_t y = 0; y < N; ++y) {
       for (int32_t x = 0; x < N; ++x) {
         const double l = pix_l(x, N, S), mm = pix_l(y, N, S), n = pix_n(l, mm);
+        if (prm->flags & ORACLE_SPAN_ATERMS) {
+          /* per-sample c_pk (section 3.4, Alg. 1: c*_pk sits INSIDE the k-sum):
+           * Sg = taper sum_k A1_k^H (Y_k phasor_k) A2_k with A_k the Jones matrices of the slot of timestep k */
+          cplx tot[4] = {0, 0, 0, 0};
+          for (int32_t t = m->time_begin; t < m->time_begin + m->n_time; ++t) {
+            const float *uvw_t = uvw + ((size_t)m->baseline * T + t) * 3;
+            cplx a1[4], a2[4], a1h[4];
+            load_jones(aterms, n_stations, N, t / prm->aterm_interval, m->station1, y, x, a1);
+            load_jones(aterms, n_stations, N, t / prm->aterm_interval, m->station2, y, x, a2);
+            mat_herm(a1, a1h);
+            for (int32_t c = m->chan_begin; c < m->chan_begin + m->n_chan; ++c) {
+              const double k = freqs[c] / ORACLE_C0;
+              const double du = (double)uvw_t[0] * k - u0;
+              const double dv = (double)uvw_t[1] * k - v0;
+              const double dw = (double)uvw_t[2] * k - w0;
+              const double phase = ORACLE_TWO_PI * (du * l + dv * mm + dw * n);
+              const cplx phasor = cos(phase) + I * sin(phase);
+              const float *y4 = vis + (((size_t)m->baseline * T + t) * C + c) * 8;
+              cplx yk[4], tmp[4], res[4];
+              for (int k4 = 0; k4 < 4; ++k4) yk[k4] = ((double)y4[2 * k4] + I * (double)y4[2 * k4 + 1]) * phasor;
+              mat_mul(a1h, yk, tmp);
+              mat_mul(tmp, a2, res);
+              for (int k4 = 0; k4 < 4; ++k4) tot[k4] += res[k4];
+            }
+          }
+          const double tp = (double)taper[(size_t)y * N + x];
+          for (int k4 = 0; k4 < 4; ++k4) sg[((size_t)k4 * N + y) * N + x] = tp * tot[k4];
+          continue;
+        }
         cplx acc[4] = {0, 0, 0, 0};
         for (int32_t t = m->time_begin; t < m->time_begin + m->n_time; ++t) {
           const float *uvw_t = uvw + ((size_t)m->baseline * T + t) * 3;
@@ -356,6 +387,21 @@ void oracle_degridder(const oracle_params *prm, const oracle_meta *meta, int64_t
       }
     for (int32_t t = m->time_begin; t < m->time_begin + m->n_time; ++t) {
       const float *uvw_t = uvw + ((size_t)m->baseline * T + t) * 3;
+      if ((prm->flags & ORACLE_SPAN_ATERMS) && t / prm->aterm_interval != m->aterm_slot) {
+        /* per-sample c_pk (Alg. 2): the corrected pixels of THIS timestep's slot */
+        for (int32_t y = 0; y < N; ++y)
+          for (int32_t x = 0; x < N; ++x) {
+            cplx a1[4], a2[4], a2h[4], pix[4], tmp[4], res[4];
+            load_jones(aterms, n_stations, N, t / prm->aterm_interval, m->station1, y, x, a1);
+            load_jones(aterms, n_stations, N, t / prm->aterm_interval, m->station2, y, x, a2);
+            const double tp = (double)taper[(size_t)y * N + x];
+            for (int k4 = 0; k4 < 4; ++k4) pix[k4] = tp * sg[((size_t)k4 * N + y) * N + x];
+            mat_herm(a2, a2h);
+            mat_mul(a1, pix, tmp);
+            mat_mul(tmp, a2h, res);
+            for (int k4 = 0; k4 < 4; ++k4) dg[((size_t)k4 * N + y) * N + x] = res[k4];
+          }
+      }
       for (int32_t c = m->chan_begin; c < m->chan_begin + m->n_chan; ++c) {
         const double k = freqs[c] / ORACLE_C0;
         const double du = (double)uvw_t[0] * k - u0;

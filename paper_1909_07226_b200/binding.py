@@ -130,7 +130,13 @@ class Plan:
         """Number of A-term slots the plan indexes (max aterm_slot + 1); cached."""
         if getattr(self, "_slots", None) is None:
             meta = self.metadata()
-            self._slots = int(meta["aterm_slot"].max()) + 1 if len(meta) else 0
+            if len(meta) == 0:
+                self._slots = 0
+            elif int(self.params.flags) & 2:      # IDG_PLAN_SPAN_ATERMS: the last timestep of a block decides
+                last = (meta["time_begin"] + meta["n_time"] - 1) // int(self.params.aterm_interval)
+                self._slots = int(last.max()) + 1
+            else:
+                self._slots = int(meta["aterm_slot"].max()) + 1
         return self._slots
 
     def subgrids(self) -> torch.Tensor:

@@ -40,7 +40,11 @@ int ensure_staging(idg_plan *pl, int32_t n_slots) {
 
 int needed_slots(const idg_plan *pl) {
   int s = 0;
-  for (const auto &m : pl->meta_host) s = m.aterm_slot + 1 > s ? m.aterm_slot + 1 : s;
+  const bool span = (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
+  for (const auto &m : pl->meta_host) {
+    const int last = span ? (m.time_begin + m.n_time - 1) / pl->prm.aterm_interval : m.aterm_slot;
+    s = last + 1 > s ? last + 1 : s;
+  }
   return s;
 }
 
@@ -108,6 +112,7 @@ int idg_degrid(const idg_plan *pl, const float *uvw_dev, const void *grid_dev,
 int idg_gridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
                        const float *taper_dev, void *subgrids_dev, void *stream) {
   if (!pl || !uvw_dev || !vis_dev || !gains_dev || !taper_dev || (!subgrids_dev && pl->P > 0)) return IDG_ERR_INVALID_ARG;
+  if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
   return launch_gridder_scalar(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)gains_dev, taper_dev,
                                (float2 *)subgrids_dev, S(stream));
 }
@@ -115,6 +120,7 @@ int idg_gridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis
 int idg_degridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *subgrids_dev, const void *gains_dev,
                          const float *taper_dev, void *vis_out_dev, void *stream) {
   if (!pl || !uvw_dev || (!subgrids_dev && pl->P > 0) || !gains_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
+  if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
   return launch_degridder_scalar(pl, uvw_dev, (const float2 *)subgrids_dev, (const float2 *)gains_dev, taper_dev,
                                  (float2 *)vis_out_dev, S(stream));
 }
@@ -122,6 +128,7 @@ int idg_degridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *s
 int idg_grid_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
                     const float *taper_dev, void *grid_dev, void *stream) {
   if (!pl || !uvw_dev || !vis_dev || !gains_dev || !taper_dev || !grid_dev) return IDG_ERR_INVALID_ARG;
+  if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
   int rc = launch_gridder_scalar(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)gains_dev, taper_dev,
                                  pl->subgrids_dev, S(stream));
   if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, -1, S(stream), 0, (pl->P + 3) / 4);
@@ -132,6 +139,7 @@ int idg_grid_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_de
 int idg_degrid_scalar(const idg_plan *pl, const float *uvw_dev, const void *grid_dev, const void *gains_dev,
                       const float *taper_dev, void *vis_out_dev, void *stream) {
   if (!pl || !uvw_dev || !grid_dev || !gains_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
+  if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
   if (pl->n_skipped > 0)
     IDG_CUDA_TRY(cudaMemsetAsync(vis_out_dev, 0, sizeof(float2) * (size_t)pl->B * pl->T * pl->C, S(stream)));
   int rc = launch_splitter(pl, (const float2 *)grid_dev, pl->subgrids_dev, S(stream), 0, -1, 1);

@@ -20,13 +20,13 @@ __device__ __forceinline__ float2 dbc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 dlo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 dhi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int CPT>
+template <int N, int NT, int CPT, bool SPAN>
 __global__ void __launch_bounds__(NT)
 degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                  const double *__restrict__ freqs, const float2 *__restrict__ subgrids,
                  const float4 *__restrict__ aterms, const float *__restrict__ taper,
                  float4 *__restrict__ vis_out, int32_t T, int32_t C, int32_t n_stations, int32_t L,
-                 double image_size, double w_step) {
+                 double image_size, double w_step, int32_t aterm_interval) {
   constexpr int NPIX = N * N;
   constexpr int CH = NPIX < kPixChunk ? NPIX : kPixChunk;
   // corrected pixels, packed in polarisation pairs like the gridder's visibilities:
@@ -46,8 +46,11 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
 
   const int groups = (n_chan + CPT - 1) / CPT;       // channel groups per timestep
   const int n_items = n_time * groups;
-  const size_t a1_off = ((size_t)m.aterm_slot * n_stations + m.station1) * NPIX;
-  const size_t a2_off = ((size_t)m.aterm_slot * n_stations + m.station2) * NPIX;
+  // IDG_PLAN_SPAN_ATERMS (NEXT-4, per-sample c_pk: Alg. 2): the block is walked slot by slot; the
+  // corrected pixels are staged with the slot's Jones matrices and only the threads whose timestep lies in
+  // that slot accumulate.  Without the flag there is one slot, m.aterm_slot.
+  const int slot_first = m.aterm_slot;
+  const int slot_last = SPAN ? (m.time_begin + n_time - 1) / aterm_interval : slot_first;
   const float2 *sg = subgrids + (size_t)blockIdx.x * 4 * NPIX;
 
   for (int item0 = 0; item0 < n_items; item0 += NT) {
@@ -70,6 +73,12 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
 #pragma unroll
     for (int c = 0; c < CPT; ++c) re01[c] = re23[c] = im01[c] = im23[c] = make_float2(0.f, 0.f);
 
+    const int my_slot = SPAN ? (m.time_begin + tl) / aterm_interval : slot_first;
+    const int n_slots = SPAN ? slot_last - slot_first + 1 : 1;      // compile-time 1 without the flag
+    for (int si = 0; si < n_slots; ++si) {
+    const int slot = slot_first + si;
+    const size_t a1_off = ((size_t)slot * n_stations + m.station1) * NPIX;
+    const size_t a2_off = ((size_t)slot * n_stations + m.station2) * NPIX;
     for (int pix0 = 0; pix0 < NPIX; pix0 += CH) {
       const int npx = min(CH, NPIX - pix0);
       __syncthreads();
@@ -104,7 +113,7 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
         s_pix[2 * i + 1] = make_float4(r0.y, r1.y, r2q.y, r3.y);
       }
       __syncthreads();
-      if (active) {
+      if (active && (!SPAN || my_slot == slot)) {
 #pragma unroll(CPT >= 8 ? 1 : 2)
         for (int i = 0; i < npx; ++i) {
           const float4 c3 = s_lmn[i];
@@ -125,6 +134,7 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
         }
       }
     }
+    }
     if (active) {
       float4 *o = vis_out + (((size_t)m.baseline * T + (m.time_begin + tl)) * C + m.chan_begin + cg) * 2;
 #pragma unroll
@@ -142,11 +152,13 @@ template <int N, int NT, int CPT>
 static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgrids,
                     const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
                     int64_t p0, int64_t np) {
-  degridder_kernel<N, NT, CPT><<<(unsigned)np, NT, 0, stream>>>(
+  const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
+  auto kern = span ? degridder_kernel<N, NT, CPT, true> : degridder_kernel<N, NT, CPT, false>;
+  kern<<<(unsigned)np, NT, 0, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, subgrids + (size_t)p0 * 4 * N * N,
       reinterpret_cast<const float4 *>(aterms),
       taper, reinterpret_cast<float4 *>(vis_out), plan->T, plan->C, plan->n_stations,
-      plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
+      plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
   IDG_CUDA_TRY(cudaGetLastError());
   return IDG_OK;
 }

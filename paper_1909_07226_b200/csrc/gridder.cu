@@ -34,13 +34,13 @@ __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int PPT, int MINB>
+template <int N, int NT, int PPT, int MINB, bool SPAN>
 __global__ void __launch_bounds__(NT, MINB)
 gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                const double *__restrict__ freqs, const float4 *__restrict__ vis,
                const float4 *__restrict__ aterms, const float *__restrict__ taper,
                float2 *__restrict__ subgrids, int32_t T, int32_t C, int32_t n_stations,
-               int32_t L, double image_size, double w_step) {
+               int32_t L, double image_size, double w_step, int32_t aterm_interval) {
   static_assert(NT * PPT == N * N, "pixels must tile the CTA exactly");
   extern __shared__ float4 g_smem[];
   float4 *s_vis = g_smem;                  // [kVisBatch][2]: (re XX, re XY, re YX, re YY), (im ...)
@@ -77,6 +77,43 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
 #pragma unroll
   for (int k = 0; k < PPT; ++k) re01[k] = re23[k] = im01[k] = im23[k] = make_float2(0.f, 0.f);
 
+  // taper * A1^H * P * A2 per pixel with the Jones matrices of one A-term slot, written pol-planar.  With
+  // IDG_PLAN_SPAN_ATERMS (NEXT-4, per-sample c_pk: section 3.4) the accumulators are flushed
+  // whenever the slot of the timestep changes, so the subgrid is the sum of the per-slot corrected parts.
+  auto flush = [&](int slot, bool accumulate) {
+    const size_t a1_off = ((size_t)slot * n_stations + m.station1) * (N * N);
+    const size_t a2_off = ((size_t)slot * n_stations + m.station2) * (N * N);
+    float2 *out = subgrids + (size_t)blockIdx.x * 4 * N * N;
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+      const int pix = tid + k * NT;
+      const float4 a01 = __ldg(&aterms[(a1_off + pix) * 2]), a23 = __ldg(&aterms[(a1_off + pix) * 2 + 1]);
+      const float4 b01 = __ldg(&aterms[(a2_off + pix) * 2]), b23 = __ldg(&aterms[(a2_off + pix) * 2 + 1]);
+      const float tp = __ldg(&taper[pix]);
+      const float2 a0 = make_float2(a01.x, a01.y), a1 = make_float2(a01.z, a01.w);
+      const float2 a2 = make_float2(a23.x, a23.y), a3 = make_float2(a23.z, a23.w);
+      const float2 b0 = make_float2(b01.x, b01.y), b1 = make_float2(b01.z, b01.w);
+      const float2 b2 = make_float2(b23.x, b23.y), b3 = make_float2(b23.z, b23.w);
+      const float2 p0 = make_float2(re01[k].x, im01[k].x), p1 = make_float2(re01[k].y, im01[k].y);
+      const float2 p2 = make_float2(re23[k].x, im23[k].x), p3 = make_float2(re23[k].y, im23[k].y);
+      const float2 t00 = cadd(cmul_conj_a(a0, p0), cmul_conj_a(a2, p2));
+      const float2 t01 = cadd(cmul_conj_a(a0, p1), cmul_conj_a(a2, p3));
+      const float2 t10 = cadd(cmul_conj_a(a1, p0), cmul_conj_a(a3, p2));
+      const float2 t11 = cadd(cmul_conj_a(a1, p1), cmul_conj_a(a3, p3));
+      float2 r[4] = {cadd(cmul(t00, b0), cmul(t01, b2)), cadd(cmul(t00, b1), cmul(t01, b3)),
+                     cadd(cmul(t10, b0), cmul(t11, b2)), cadd(cmul(t10, b1), cmul(t11, b3))};
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        float2 v = make_float2(tp * r[q].x, tp * r[q].y);
+        if (SPAN && accumulate) { const float2 o = out[q * N * N + pix]; v.x += o.x; v.y += o.y; }
+        out[q * N * N + pix] = v;
+      }
+      if (SPAN) re01[k] = re23[k] = im01[k] = im23[k] = make_float2(0.f, 0.f);
+    }
+  };
+  int cur_slot = m.aterm_slot;
+  bool flushed = false;
+
   const int tb_max = n_chan >= kVisBatch ? 1 : kVisBatch / n_chan;  // timesteps per batch
   const float *uvw_b = uvw + (size_t)m.baseline * T * 3;
 
@@ -105,6 +142,10 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
       __syncthreads();
 
       for (int tl = 0; tl < tb; ++tl) {
+        if (SPAN) {
+          const int slot = (m.time_begin + t0 + tl) / aterm_interval;
+          if (slot != cur_slot) { flush(cur_slot, flushed); flushed = true; cur_slot = slot; }
+        }
         const float4 tu = s_t[2 * tl], tbs = s_t[2 * tl + 1];
         float pidx[PPT], base[PPT];
 #pragma unroll
@@ -135,47 +176,20 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
     }
   }
 
-  // epilogue: taper * A1^H * P * A2 per pixel, written pol-planar
-  const size_t a1_off = ((size_t)m.aterm_slot * n_stations + m.station1) * (N * N);
-  const size_t a2_off = ((size_t)m.aterm_slot * n_stations + m.station2) * (N * N);
-  float2 *out = subgrids + (size_t)blockIdx.x * 4 * N * N;
-#pragma unroll
-  for (int k = 0; k < PPT; ++k) {
-    const int pix = tid + k * NT;
-    const float4 a01 = __ldg(&aterms[(a1_off + pix) * 2]), a23 = __ldg(&aterms[(a1_off + pix) * 2 + 1]);
-    const float4 b01 = __ldg(&aterms[(a2_off + pix) * 2]), b23 = __ldg(&aterms[(a2_off + pix) * 2 + 1]);
-    const float tp = __ldg(&taper[pix]);
-    const float2 a0 = make_float2(a01.x, a01.y), a1 = make_float2(a01.z, a01.w);
-    const float2 a2 = make_float2(a23.x, a23.y), a3 = make_float2(a23.z, a23.w);
-    const float2 b0 = make_float2(b01.x, b01.y), b1 = make_float2(b01.z, b01.w);
-    const float2 b2 = make_float2(b23.x, b23.y), b3 = make_float2(b23.z, b23.w);
-    const float2 p0 = make_float2(re01[k].x, im01[k].x), p1 = make_float2(re01[k].y, im01[k].y);
-    const float2 p2 = make_float2(re23[k].x, im23[k].x), p3 = make_float2(re23[k].y, im23[k].y);
-    const float2 t00 = cadd(cmul_conj_a(a0, p0), cmul_conj_a(a2, p2));
-    const float2 t01 = cadd(cmul_conj_a(a0, p1), cmul_conj_a(a2, p3));
-    const float2 t10 = cadd(cmul_conj_a(a1, p0), cmul_conj_a(a3, p2));
-    const float2 t11 = cadd(cmul_conj_a(a1, p1), cmul_conj_a(a3, p3));
-    float2 r0 = cadd(cmul(t00, b0), cmul(t01, b2));
-    float2 r1 = cadd(cmul(t00, b1), cmul(t01, b3));
-    float2 r2 = cadd(cmul(t10, b0), cmul(t11, b2));
-    float2 r3 = cadd(cmul(t10, b1), cmul(t11, b3));
-    out[0 * N * N + pix] = make_float2(tp * r0.x, tp * r0.y);
-    out[1 * N * N + pix] = make_float2(tp * r1.x, tp * r1.y);
-    out[2 * N * N + pix] = make_float2(tp * r2.x, tp * r2.y);
-    out[3 * N * N + pix] = make_float2(tp * r3.x, tp * r3.y);
-  }
+  flush(cur_slot, flushed);
 }
 
 template <int N, int NT, int PPT, int MINB>
 static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
                     const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
   constexpr size_t smem = sizeof(float4) * (kVisBatch * 4 + N * N) + sizeof(float) * kMaxChan;
-  auto kern = gridder_kernel<N, NT, PPT, MINB>;
+  const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
+  auto kern = span ? gridder_kernel<N, NT, PPT, MINB, true> : gridder_kernel<N, NT, PPT, MINB, false>;
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(unsigned)np, NT, smem, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
       reinterpret_cast<const float4 *>(aterms), taper, subgrids + (size_t)p0 * 4 * N * N, plan->T, plan->C,
-      plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step);
+      plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
   IDG_CUDA_TRY(cudaGetLastError());
   return IDG_OK;
 }

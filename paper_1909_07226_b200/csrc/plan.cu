@@ -18,7 +18,7 @@
 namespace idg {
 
 struct PlanConst {
-  int32_t B, T, C, N, L, max_timesteps, max_channels, aterm_interval, force;
+  int32_t B, T, C, N, L, max_timesteps, max_channels, aterm_interval, force, span;
   double budget, w_step;
 };
 
@@ -54,7 +54,7 @@ __device__ void walk_baseline(const PlanConst pc, const float *__restrict__ uvw_
       double umin = 0, umax = 0, vmin = 0, vmax = 0;
       int32_t wi0 = 0;
       while (t1 < pc.T && t1 - t0 < pc.max_timesteps &&
-             t1 / pc.aterm_interval == t0 / pc.aterm_interval) {
+             (pc.span || t1 / pc.aterm_interval == t0 / pc.aterm_interval)) {
         int32_t wi = 0;
         if (pc.w_step > 0.0)
           wi = (int32_t)floor(__ddiv_rn(__dmul_rn((double)uvw_b[3 * t1 + 2], k_mid), pc.w_step));
@@ -122,6 +122,7 @@ int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *
   pc.B = B; pc.T = T; pc.C = C; pc.N = prm.subgrid_size; pc.L = prm.grid_size;
   pc.max_timesteps = prm.max_timesteps; pc.max_channels = prm.max_channels;
   pc.aterm_interval = prm.aterm_interval; pc.force = (prm.flags & IDG_PLAN_FORCE_BLOCKS) != 0;
+  pc.span = (prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
   pc.budget = (double)(prm.subgrid_size - prm.kernel_size);
   pc.w_step = prm.w_step;
   // pixel scale per channel: (f / c0) * S, two roundings in this order (host, no contraction:

@@ -34,6 +34,7 @@ SPEED_OF_LIGHT = 299792458.0
 EARTH_ROTATION_RAD_S = 7.2921150e-5
 
 FLAG_FORCE_BLOCKS = 1
+FLAG_SPAN_ATERMS = 2
 
 
 @dataclasses.dataclass

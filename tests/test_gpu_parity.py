@@ -512,3 +512,39 @@ def test_ska_full_size_sampled():
     w = synth.make_workload("ska", device="cuda")            # generated on the GPU (seconds), checked from a host copy
     host = dataclasses.replace(w, uvw=w.uvw.cpu(), vis=w.vis.cpu(), aterms=w.aterms.cpu(), taper=w.taper.cpu())
     assert _sampled_full_size_check(host, 24, 31) > 250000
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4: per-sample c_pk -- blocks that span A-term slots (IDG_PLAN_SPAN_ATERMS)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("a_int", [1, 5])
+def test_spanning_blocks_per_sample_aterms(a_int):
+    w = synth.make_workload("tiny", aterm_interval=a_int)
+    prm = dataclasses.replace(w.params, flags=synth.FLAG_SPAN_ATERMS, w_step=150.0)
+    plan, wc, meta = _plan_both(w, prm)                                  # plan bit-exact with the flag
+    last = (meta["time_begin"] + meta["n_time"] - 1) // a_int
+    assert np.any(last > meta["aterm_slot"])
+    d = _np(w)
+    L = prm.grid_size
+    ref = orc.grid(prm, meta, d["uvw"], d["freqs"], d["vis"], d["aterms"], d["taper"])
+    g = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    idg.idg_grid(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, g)
+    torch.cuda.synchronize()
+    assert H.rel_l2(g.cpu().numpy(), ref) < TOL
+    ref_sub = orc.gridder(prm, meta, d["uvw"], d["freqs"], d["vis"], d["aterms"], d["taper"])
+    sub = torch.zeros(ref_sub.shape, dtype=torch.complex64, device="cuda")
+    idg.idg_gridder(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, sub)
+    torch.cuda.synchronize()
+    got = sub.cpu().numpy()
+    assert max(H.rel_l2(got[p], ref_sub[p]) for p in range(len(meta))) < TOL
+    model = ref.astype(np.complex64)
+    refv = orc.degrid(prm, meta, d["uvw"], d["freqs"], model.astype(np.complex128), d["aterms"], d["taper"], w.B)
+    out = torch.zeros_like(wc.vis)
+    idg.idg_degrid(plan, wc.uvw, torch.from_numpy(model).cuda(), wc.aterms, wc.taper, out)
+    torch.cuda.synchronize()
+    assert H.rel_l2(out.cpu().numpy(), refv) < TOL
+    # the scalar kernels know per-block gains only and must refuse such a plan
+    with pytest.raises(idg.IdgError):
+        idg.idg_grid_scalar(plan, wc.uvw, wc.vis[..., 0].contiguous(), wc.aterms[..., 0].contiguous(), wc.taper,
+                            torch.zeros((L, L), dtype=torch.complex64, device="cuda"))
