@@ -20,7 +20,7 @@ __device__ __forceinline__ float2 dbc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 dlo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 dhi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int CPT, bool SPAN>
+template <int N, int NT, int CPT, bool SPAN, bool SPLIT>
 __global__ void __launch_bounds__(NT)
 degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                  const double *__restrict__ freqs, const float2 *__restrict__ subgrids,
@@ -33,6 +33,10 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
   // (re XX, re XY, re YX, re YY), (im ...) -- one FFMA2 updates two polarisations
   __shared__ float4 s_pix[CH * 2];
   __shared__ float4 s_lmn[CH];       // l, m, n', unused
+  // partial sums of the SPLIT reduction: NT CPT 8 floats at most; the pixel staging area is reused when it is
+  // large enough (N >= 24), N = 16 gets its own
+  constexpr bool kOwnRed = SPLIT && (CH * 8 < NT * CPT * 8);
+  __shared__ float s_red_own[kOwnRed ? NT * CPT * 8 : 1];
 
   const int tid = threadIdx.x;
   const idg_subgrid_meta m = meta[blockIdx.x];
@@ -53,9 +57,14 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
   const int slot_last = SPAN ? (m.time_begin + n_time - 1) / aterm_interval : slot_first;
   const float2 *sg = subgrids + (size_t)blockIdx.x * 4 * NPIX;
 
+  // SPLIT (plans whose largest block fills at most half the CTA, e.g. A-terms refreshed every few timesteps): the
+  // threads are arranged as G groups x n_items; group g sums the pixels g, g + G, ... and the partial sums are
+  // reduced through shared memory at the end, so that short blocks still use the whole CTA.
+  const int G = SPLIT ? max(1, min(8, NT / max(n_items, 1))) : 1;
+  const int grp = SPLIT ? tid / max(n_items, 1) : 0;
   for (int item0 = 0; item0 < n_items; item0 += NT) {
-    const int item = item0 + tid;
-    const bool active = item < n_items;
+    const int item = SPLIT ? tid - grp * n_items : item0 + tid;
+    const bool active = SPLIT ? grp < G : item < n_items;
     const int tl = active ? item / groups : 0;
     const int cg = active ? (item - tl * groups) * CPT : 0;
     const float *p = uvw + ((size_t)m.baseline * T + (m.time_begin + tl)) * 3;
@@ -115,7 +124,7 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
       __syncthreads();
       if (active && (!SPAN || my_slot == slot)) {
 #pragma unroll(CPT >= 8 ? 1 : 2)
-        for (int i = 0; i < npx; ++i) {
+        for (int i = grp; i < npx; i += G) {
           const float4 c3 = s_lmn[i];
           const float4 qr = s_pix[2 * i], qi = s_pix[2 * i + 1];
           const float pidx = fmaf(u, c3.x, fmaf(v, c3.y, w * c3.z));
@@ -135,7 +144,30 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
       }
     }
     }
-    if (active) {
+    if (SPLIT && G > 1) {
+      float *red = kOwnRed ? s_red_own : reinterpret_cast<float *>(s_pix);   // [G - 1][n_items][CPT][8]
+      __syncthreads();
+      if (active && grp > 0) {
+        float *r = red + ((size_t)(grp - 1) * n_items + item) * (CPT * 8);
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) {
+          r[8 * c + 0] = re01[c].x; r[8 * c + 1] = re01[c].y; r[8 * c + 2] = re23[c].x; r[8 * c + 3] = re23[c].y;
+          r[8 * c + 4] = im01[c].x; r[8 * c + 5] = im01[c].y; r[8 * c + 6] = im23[c].x; r[8 * c + 7] = im23[c].y;
+        }
+      }
+      __syncthreads();
+      if (active && grp == 0) {
+        for (int g = 1; g < G; ++g) {
+          const float *r = red + ((size_t)(g - 1) * n_items + item) * (CPT * 8);
+#pragma unroll
+          for (int c = 0; c < CPT; ++c) {
+            re01[c].x += r[8 * c + 0]; re01[c].y += r[8 * c + 1]; re23[c].x += r[8 * c + 2]; re23[c].y += r[8 * c + 3];
+            im01[c].x += r[8 * c + 4]; im01[c].y += r[8 * c + 5]; im23[c].x += r[8 * c + 6]; im23[c].y += r[8 * c + 7];
+          }
+        }
+      }
+    }
+    if (active && grp == 0) {
       float4 *o = vis_out + (((size_t)m.baseline * T + (m.time_begin + tl)) * C + m.chan_begin + cg) * 2;
 #pragma unroll
       for (int c = 0; c < CPT; ++c) {
@@ -148,12 +180,12 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
   }
 }
 
-template <int N, int NT, int CPT>
+template <int N, int NT, int CPT, bool SPLIT = false>
 static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgrids,
                     const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
                     int64_t p0, int64_t np) {
   const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
-  auto kern = span ? degridder_kernel<N, NT, CPT, true> : degridder_kernel<N, NT, CPT, false>;
+  auto kern = span ? degridder_kernel<N, NT, CPT, true, SPLIT> : degridder_kernel<N, NT, CPT, false, SPLIT>;
   kern<<<(unsigned)np, NT, 0, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, subgrids + (size_t)p0 * 4 * N * N,
       reinterpret_cast<const float4 *>(aterms),
@@ -175,6 +207,11 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
   if (mc >= 8 && plan->max_n_time * ((mc + 7) / 8) >= 128) cpt = 8;
   const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
   const bool small = items <= 128;
+  if (items <= 64 && cpt <= 4 && N >= 24) {   // short blocks: split the pixels over thread groups (measured: no gain at N = 16)
+    if (cpt == 4) return launch_k<N, 128, 4, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    if (cpt == 2) return launch_k<N, 128, 2, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    return launch_k<N, 128, 1, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+  }
 #define IDG_DG(CPT_)                                                                         \
   return small ? launch_k<N, 128, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np) \
                : launch_k<N, 256, CPT_>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np)
