@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="lofar", choices=["tiny", "lofar", "ska"])
+    ap.add_argument("--workload", default="lofar", choices=["tiny", "lofar", "ska", "paper"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -55,6 +55,7 @@ WORKLOAD_NAMES = {
     "tiny": "configs[0] tiny: 8 stations, 32 x 10 s, 4 ch, N=24, L=256",
     "lofar": "configs[1] LOFAR-HBA-like: 48 stations (1128 baselines), 256 x 2 s, 16 ch, N=32, L=2048",
     "ska": "configs[2]+[3] SKA-low-like: 128 stations (8128 baselines), 1024 x 1 s, 16 ch, N=32, L=8192",
+    "paper": "context: the paper's simulation shape (55 stations, 3122 x 10 s, 20 ch, N=48, L=2048; PAPER.md:445,471-473)",
 }
 
 
@@ -330,6 +331,7 @@ def run_b200(args):
     touched_px = int(np.count_nonzero(np.cumsum(np.cumsum(diff, axis=0), axis=1)[:L, :L]))
     touched = 2 * 32.0 * touched_px                      # read + write of every touched 4-pol grid pixel
     extra = {
+        "correlations_per_s": 4.0 * value * 1e6,      # 4 polarisations per visibility (BASELINE.json's "0.5 G" reading)
         "plan_ms": plan_ms, "n_subgrids": P, "n_vis_per_rank": planned, "n_skipped": skipped,
         "stage_ms": stage_ms,
         "grid_mvis_s": planned / ((stage_ms["gridder"] + stage_ms["subgrid_fft"] + stage_ms["adder"]) * 1e-3) / 1e6,

@@ -242,6 +242,11 @@ _CONFIG_TABLE = {
                   S=0.05, max_t=128, max_c=16, a_int=64, w_step=0.0, n_src=100, flux=(0.01, 10.0), inner=0.6),
     "ska": dict(idx=2, lat=-26.8, dec=-40.0, T=1024, dt=1.0, f0=100e6, df=100e3, C=16, N=32, L=8192,
                 S=0.16, max_t=256, max_c=16, a_int=32, w_step=256.0, n_src=100, flux=(0.01, 10.0), inner=0.6),
+    # context only: the shape of the paper's simulation (section 5.1/5.3): 55 stations,
+    # baselines out to 84 km, 3122 x 10 s, 20 channels 130-132 MHz, 2048^2 image with 1" cells, 48 x 48 subgrids
+    "paper": dict(idx=5, lat=52.9, dec=50.0, T=3122, dt=10.0, f0=130e6, df=100e3, C=20, N=48, L=2048,
+                  S=2048 * math.pi / (180.0 * 3600.0), max_t=256, max_c=32, a_int=256, w_step=0.0, n_src=1,
+                  flux=None, inner=0.2),
     "sweep": dict(idx=4, lat=52.9, dec=50.0, T=1024, dt=2.0, f0=140e6, df=195e3, C=64, N=32, L=2048,
                   S=0.05, max_t=128, max_c=16, a_int=64, w_step=0.0, n_src=100, flux=(0.01, 10.0), inner=0.6),
 }
@@ -256,6 +261,8 @@ def _stations(name: str, rng) -> np.ndarray:
         return layout_core_plus_outliers(rng, 36, 2500.0, 12, 2500.0, 20000.0)
     if name == "ska":
         return layout_log_radial(rng, 128, 50.0, 35000.0)
+    if name == "paper":
+        return layout_log_radial(rng, 55, 60.0, 42000.0)
     raise KeyError(name)
 
 
