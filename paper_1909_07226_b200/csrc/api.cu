@@ -93,6 +93,16 @@ static int finish_plan(idg_plan *pl, const double *freqs_host, cudaStream_t stre
     pl->max_n_time = std::max(pl->max_n_time, m.n_time);
     pl->max_n_chan = std::max(pl->max_n_chan, m.n_chan);
   }
+  // fraction of idle channel slots in the degridder if every thread owns cpt = 1, 2, 4, 8 channels of a timestep
+  for (int k = 0; k < 4; ++k) {
+    const int cpt = 1 << k;
+    double used = 0.0, slots = 0.0;
+    for (const auto &m : pl->meta_host) {
+      used += (double)m.n_time * m.n_chan;
+      slots += (double)m.n_time * ((m.n_chan + cpt - 1) / cpt) * cpt;
+    }
+    pl->dg_waste[k] = slots > 0.0 ? (float)(1.0 - used / slots) : 0.f;
+  }
   pl->uniform_dkd = 0.f;
   if (pl->C >= 2) {
     const double df = freqs_host[1] - freqs_host[0];

@@ -28,6 +28,7 @@ struct idg_plan {
   int32_t B = 0, T = 0, C = 0, n_stations = 0;
   int64_t P = 0, n_planned = 0, n_skipped = 0;
   int32_t max_n_time = 0, max_n_chan = 0;
+  float dg_waste[4] = {0.f, 0.f, 0.f, 0.f};   // degridder: idle channel slots if threads own 1, 2, 4, 8 channels
   float uniform_dkd = 0.f;            // 2 pi df / c0 when the channels are equally spaced, else 0 (scalar.cu)
   std::vector<idg_subgrid_meta> meta_host;
   idg_subgrid_meta *meta_dev = nullptr;

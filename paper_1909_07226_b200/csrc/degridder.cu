@@ -205,6 +205,8 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
   // largest block still fills a 128-thread CTA
   int cpt = mc >= 4 ? 4 : (mc >= 2 ? 2 : 1);
   if (mc >= 8 && plan->max_n_time * ((mc + 7) / 8) >= 128) cpt = 8;
+  // plans that mix channel-group sizes (a 20-channel band cut into 16 + 4): do not idle more than 5 % of the slots
+  while (cpt > 1 && plan->dg_waste[cpt == 8 ? 3 : (cpt == 4 ? 2 : 1)] > 0.05f) cpt /= 2;
   const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
   const bool small = items <= 128;
   if (items <= 64 && cpt <= 4 && N >= 24) {   // short blocks: split the pixels over thread groups (measured: no gain at N = 16)
