@@ -548,3 +548,24 @@ def test_spanning_blocks_per_sample_aterms(a_int):
     with pytest.raises(idg.IdgError):
         idg.idg_grid_scalar(plan, wc.uvw, wc.vis[..., 0].contiguous(), wc.aterms[..., 0].contiguous(), wc.taper,
                             torch.zeros((L, L), dtype=torch.complex64, device="cuda"))
+
+
+def test_calls_run_on_the_callers_stream(tiny_case):
+    """The library is asynchronous on the stream it is given and never synchronises it: work queued on a side
+    stream behind a long-running kernel must not have run until that stream is waited on, and must be right then."""
+    c = tiny_case
+    L = c["prm"].grid_size
+    side = torch.cuda.Stream()
+    g = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    ref = torch.zeros_like(g)
+    idg.idg_grid(c["plan"], c["wc"].uvw, c["wc"].vis, c["wc"].aterms, c["wc"].taper, ref)      # default stream
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        torch.cuda._sleep(200_000_000)                                   # ~0.1 s of spinning on the side stream
+        idg.idg_grid(c["plan"], c["wc"].uvw, c["wc"].vis, c["wc"].aterms, c["wc"].taper, g, stream=side)
+        done = torch.cuda.Event()
+        done.record(side)
+    assert not done.query()                                              # the call returned without waiting
+    side.synchronize()
+    # the adder's per-tile reductions land in any order, so equal up to FP32 summation order only
+    assert H.rel_l2(g.cpu().numpy(), ref.cpu().numpy()) < 1e-6
