@@ -20,7 +20,7 @@ __device__ __forceinline__ float2 dbc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 dlo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 dhi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int CPT, bool SPAN, bool SPLIT>
+template <int N, int NT, int CPT, bool SPAN, bool SPLIT, bool ONECHAN = false>
 __global__ void __launch_bounds__(NT)
 degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                  const double *__restrict__ freqs, const float2 *__restrict__ subgrids,
@@ -127,12 +127,13 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
         for (int i = grp; i < npx; i += G) {
           const float4 c3 = s_lmn[i];
           const float4 qr = s_pix[2 * i], qi = s_pix[2 * i + 1];
-          const float pidx = fmaf(u, c3.x, fmaf(v, c3.y, w * c3.z));
+          // single-channel plans: kd = 0 exactly, the phase is `base` alone
+          const float pidx = ONECHAN ? 0.f : fmaf(u, c3.x, fmaf(v, c3.y, w * c3.z));
           const float base = fmaf(bu, c3.x, fmaf(bv, c3.y, bw * c3.z));
 #pragma unroll
           for (int c = 0; c < CPT; ++c) {
             float s, co;
-            __sincosf(fmaf(pidx, kd[c], base), &s, &co);
+            __sincosf(ONECHAN ? base : fmaf(pidx, kd[c], base), &s, &co);
             const float ns = -s;
             // (re + i im) += (qr + i qi)(co - i s): the conjugate phasor of the gridder
             re01[c] = ffma2(dlo2(qr), dbc2(co), re01[c]); re01[c] = ffma2(dlo2(qi), dbc2(s), re01[c]);
@@ -185,7 +186,10 @@ static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgri
                     const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
                     int64_t p0, int64_t np) {
   const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
-  auto kern = span ? degridder_kernel<N, NT, CPT, true, SPLIT> : degridder_kernel<N, NT, CPT, false, SPLIT>;
+  const bool one = CPT == 1 && !span && plan->max_n_chan == 1;
+  auto kern = span ? degridder_kernel<N, NT, CPT, true, SPLIT>
+                   : (one ? degridder_kernel<N, NT, (CPT == 1 ? 1 : CPT), false, SPLIT, CPT == 1>
+                          : degridder_kernel<N, NT, CPT, false, SPLIT>);
   kern<<<(unsigned)np, NT, 0, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, subgrids + (size_t)p0 * 4 * N * N,
       reinterpret_cast<const float4 *>(aterms),

@@ -34,7 +34,7 @@ __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int PPT, int MINB, bool SPAN>
+template <int N, int NT, int PPT, int MINB, bool SPAN, bool ONECHAN>
 __global__ void __launch_bounds__(NT, MINB)
 gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                const double *__restrict__ freqs, const float4 *__restrict__ vis,
@@ -141,6 +141,28 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
       }
       __syncthreads();
 
+      if (ONECHAN) {
+        // plans with one channel per subgrid: k_mid is that channel, kd = 0 exactly and the phase is `base` alone;
+        // the timesteps take the place of the channel loop (3 FMA + sin/cos + 16 FMA per pair, no per-timestep set-up)
+        float ql[PPT], qm[PPT], qn[PPT];
+#pragma unroll
+        for (int k = 0; k < PPT; ++k) { const float4 q = s_lmn[tid + k * NT]; ql[k] = q.x; qm[k] = q.y; qn[k] = q.z; }
+#pragma unroll 4
+        for (int tl = 0; tl < tb; ++tl) {
+          const float4 tbs = s_t[2 * tl + 1];
+          const float4 vr = s_vis[2 * tl], vi = s_vis[2 * tl + 1];
+#pragma unroll
+          for (int k = 0; k < PPT; ++k) {
+            float s, co;
+            __sincosf(fmaf(tbs.x, ql[k], fmaf(tbs.y, qm[k], tbs.z * qn[k])), &s, &co);
+            const float ns = -s;
+            re01[k] = ffma2(lo2(vr), bc2(co), re01[k]); re01[k] = ffma2(lo2(vi), bc2(ns), re01[k]);
+            re23[k] = ffma2(hi2(vr), bc2(co), re23[k]); re23[k] = ffma2(hi2(vi), bc2(ns), re23[k]);
+            im01[k] = ffma2(lo2(vr), bc2(s), im01[k]);  im01[k] = ffma2(lo2(vi), bc2(co), im01[k]);
+            im23[k] = ffma2(hi2(vr), bc2(s), im23[k]);  im23[k] = ffma2(hi2(vi), bc2(co), im23[k]);
+          }
+        }
+      } else
       for (int tl = 0; tl < tb; ++tl) {
         if (SPAN) {
           const int slot = (m.time_begin + t0 + tl) / aterm_interval;
@@ -184,7 +206,10 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, c
                     const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
   constexpr size_t smem = sizeof(float4) * (kVisBatch * 4 + N * N) + sizeof(float) * kMaxChan;
   const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
-  auto kern = span ? gridder_kernel<N, NT, PPT, MINB, true> : gridder_kernel<N, NT, PPT, MINB, false>;
+  // single-channel plans without the span flag take the ONECHAN instance
+  const bool one = !span && plan->max_n_chan == 1;
+  auto kern = span ? gridder_kernel<N, NT, PPT, MINB, true, false>
+                   : (one ? gridder_kernel<N, NT, PPT, MINB, false, true> : gridder_kernel<N, NT, PPT, MINB, false, false>);
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(unsigned)np, NT, smem, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
