@@ -48,6 +48,37 @@ int needed_slots(const idg_plan *pl) {
   return s;
 }
 
+// The host-buffer calls overlap the PCIe copies with the kernels: the baselines are cut into kHostChunks
+// contiguous ranges (the metadata is sorted by baseline, so a range of baselines is a range of subgrids and a
+// contiguous slice of vis); uploads run on the plan's copy stream, kernels on the caller's stream, events
+// order them.  Gridding: chunk k is gridded while chunk k+1 and then the grid itself are uploaded; the adder
+// runs once at the end.  Degridding: chunk k's visibilities travel back while chunk k+1 is predicted.
+struct HostChunk { int32_t b0, b1; int64_t p0, p1; };
+
+int ensure_host_pipeline(idg_plan *pl) {
+  if (!pl->h_copy_stream) IDG_CUDA_TRY(cudaStreamCreateWithFlags(&pl->h_copy_stream, cudaStreamNonBlocking));
+  for (auto &e : pl->h_ev_in) if (!e) IDG_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  for (auto &e : pl->h_ev_out) if (!e) IDG_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  return IDG_OK;
+}
+
+std::vector<HostChunk> host_chunks(const idg_plan *pl) {
+  std::vector<HostChunk> out;
+  const int n = std::min<int>(idg_plan::kHostChunks, pl->B);
+  int64_t p = 0;
+  for (int k = 0; k < n; ++k) {
+    HostChunk c;
+    c.b0 = (int32_t)((int64_t)pl->B * k / n);
+    c.b1 = (int32_t)((int64_t)pl->B * (k + 1) / n);
+    c.p0 = p;
+    while (p < pl->P && pl->meta_host[(size_t)p].baseline < c.b1) ++p;
+    c.p1 = p;
+    out.push_back(c);
+  }
+  return out;
+}
+
+
 }  // namespace
 
 extern "C" {
@@ -148,36 +179,6 @@ int idg_degrid_scalar(const idg_plan *pl, const float *uvw_dev, const void *grid
     rc = launch_degridder_scalar(pl, uvw_dev, pl->subgrids_dev, (const float2 *)gains_dev, taper_dev,
                                  (float2 *)vis_out_dev, S(stream));
   return rc;
-}
-
-// The host-buffer calls overlap the PCIe copies with the kernels: the baselines are cut into kHostChunks
-// contiguous ranges (the metadata is sorted by baseline, so a range of baselines is a range of subgrids and a
-// contiguous slice of vis); uploads run on the plan's copy stream, kernels on the caller's stream, events
-// order them.  Gridding: chunk k is gridded while chunk k+1 and then the grid itself are uploaded; the adder
-// runs once at the end.  Degridding: chunk k's visibilities travel back while chunk k+1 is predicted.
-struct HostChunk { int32_t b0, b1; int64_t p0, p1; };
-
-static int ensure_host_pipeline(idg_plan *pl) {
-  if (!pl->h_copy_stream) IDG_CUDA_TRY(cudaStreamCreateWithFlags(&pl->h_copy_stream, cudaStreamNonBlocking));
-  for (auto &e : pl->h_ev_in) if (!e) IDG_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-  for (auto &e : pl->h_ev_out) if (!e) IDG_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-  return IDG_OK;
-}
-
-static std::vector<HostChunk> host_chunks(const idg_plan *pl) {
-  std::vector<HostChunk> out;
-  const int n = std::min<int>(idg_plan::kHostChunks, pl->B);
-  int64_t p = 0;
-  for (int k = 0; k < n; ++k) {
-    HostChunk c;
-    c.b0 = (int32_t)((int64_t)pl->B * k / n);
-    c.b1 = (int32_t)((int64_t)pl->B * (k + 1) / n);
-    c.p0 = p;
-    while (p < pl->P && pl->meta_host[(size_t)p].baseline < c.b1) ++p;
-    c.p1 = p;
-    out.push_back(c);
-  }
-  return out;
 }
 
 int idg_grid_host(idg_plan *pl, const float *uvw_host, const void *vis_host,
