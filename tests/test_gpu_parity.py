@@ -569,3 +569,38 @@ def test_calls_run_on_the_callers_stream(tiny_case):
     side.synchronize()
     # the adder's per-tile reductions land in any order, so equal up to FP32 summation order only
     assert H.rel_l2(g.cpu().numpy(), ref.cpu().numpy()) < 1e-6
+
+
+def test_error_paths_with_a_device(tiny_case):
+    """Bad arguments come back as status codes (IdgError in the binding), never as a crash."""
+    c = tiny_case
+    w, prm = c["w"], c["prm"]
+    # metadata that does not fit the arrays or the grid
+    bad = c["meta"].copy()
+    bad["x0"][0] = prm.grid_size                      # subgrid outside the grid
+    with pytest.raises(idg.IdgError, match="metadata does not match"):
+        idg.idg_plan_from_metadata(prm, bad, w.freqs, w.B, w.T, w.n_stations)
+    bad = c["meta"].copy()
+    bad["time_begin"][0] = w.T                        # block beyond the last timestep
+    with pytest.raises(idg.IdgError, match="metadata does not match"):
+        idg.idg_plan_from_metadata(prm, bad, w.freqs, w.B, w.T, w.n_stations)
+    # unsupported subgrid size and bad parameters
+    with pytest.raises(idg.IdgError, match="subgrid size"):
+        idg.idg_plan_create(dataclasses.replace(prm, subgrid_size=20), c["wc"].uvw, w.freqs, w.baselines, w.n_stations)
+    with pytest.raises(idg.IdgError, match="invalid argument"):
+        idg.idg_plan_create(dataclasses.replace(prm, max_channels=3), c["wc"].uvw, w.freqs, w.baselines, w.n_stations)
+    with pytest.raises(idg.IdgError, match="invalid argument"):
+        idg.idg_plan_create(dataclasses.replace(prm, flags=8), c["wc"].uvw, w.freqs, w.baselines, w.n_stations)
+    # too few A-term slots, wrong shapes, host tensors where device tensors are expected
+    L = prm.grid_size
+    g = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    with pytest.raises(idg.IdgError, match="slots"):
+        idg.idg_grid(c["plan"], c["wc"].uvw, c["wc"].vis, c["wc"].aterms[:1].contiguous(), c["wc"].taper, g)
+    with pytest.raises(idg.IdgError, match="grid shape"):
+        idg.idg_grid(c["plan"], c["wc"].uvw, c["wc"].vis, c["wc"].aterms, c["wc"].taper, g[:, :-1].contiguous())
+    with pytest.raises(idg.IdgError, match="CUDA tensor"):
+        idg.idg_grid(c["plan"], c["wc"].uvw.cpu(), c["wc"].vis, c["wc"].aterms, c["wc"].taper, g)
+    # the C ABI itself rejects too few slots on the host path
+    with pytest.raises(idg.IdgError):
+        idg.idg_subgrid_fft(c["plan"], c["plan"].subgrids(), 0)           # direction must be -1 or +1
+    assert torch.all(g == 0)
