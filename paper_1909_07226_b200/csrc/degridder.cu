@@ -21,7 +21,7 @@ __device__ __forceinline__ float2 dlo2(float4 v) { return make_float2(v.x, v.y);
 __device__ __forceinline__ float2 dhi2(float4 v) { return make_float2(v.z, v.w); }
 
 template <int N, int NT, int CPT, bool SPAN, bool SPLIT, bool ONECHAN = false>
-__global__ void __launch_bounds__(NT)
+__global__ void __launch_bounds__(NT, NT == 128 ? 4 : 2)
 degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                  const double *__restrict__ freqs, const float2 *__restrict__ subgrids,
                  const float4 *__restrict__ aterms, const float *__restrict__ taper,
