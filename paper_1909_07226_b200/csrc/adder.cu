@@ -7,12 +7,12 @@
 // Subgrids overlap ("subgrids may overlap"), heavily near the uv origin.  Instead
 // of one atomic per subgrid pixel, the plan buckets the subgrids by the 128 x 8 grid tiles they
 // touch (stable in the subgrid index; wide tiles so that a subgrid row is rarely split between two
-// work items -- a split 32-byte sector is fetched from HBM twice).  One work item = one tile and up to kAdderChunk of its
-// subgrids: the CTA gathers their overlapping parts into registers in plan order and adds the
-// tile to the grid once, with one vector reduction (red.global.add.v2.f32) per pixel.  Every
-// subgrid element is read exactly once; the grid sees one reduction per (work item, pixel)
-// instead of one per (subgrid, pixel).  Long lists (the uv core) are split over several work
-// items so no CTA becomes the tail.
+// work items -- a split 32-byte sector is fetched from HBM twice).  One work item = one tile and
+// up to kAdderChunk of its subgrids: the CTA sums their overlapping parts into a shared-memory
+// copy of the tile in plan order and adds the tile to the grid once, with one vector reduction
+// (red.global.add.v2.f32) per touched pixel.  Every subgrid element is read exactly once; the
+// grid sees one reduction per (work item, pixel) instead of one per (subgrid, pixel).  Long lists
+// (the uv core) are split over several work items so no CTA becomes the tail.
 #include <algorithm>
 
 #include "common.cuh"
