@@ -27,25 +27,25 @@
 
 namespace idg {
 
-constexpr int kVisBatch = 256;   // visibilities staged per batch (2 float4 each = 8 KB)
 constexpr int kMaxChan = 256;    // max channels per subgrid
 
 __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int PPT, int MINB, bool SPAN, bool ONECHAN>
+template <int N, int NT, int PPT, int MINB, int VB, int TB, bool SPAN, bool ONECHAN>
 __global__ void __launch_bounds__(NT, MINB)
 gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                const double *__restrict__ freqs, const float4 *__restrict__ vis,
                const float4 *__restrict__ aterms, const float *__restrict__ taper,
                float2 *__restrict__ subgrids, int32_t T, int32_t C, int32_t n_stations,
                int32_t L, double image_size, double w_step, int32_t aterm_interval) {
+  constexpr int vis_batch = VB, time_batch = TB;
   static_assert(NT * PPT == N * N, "pixels must tile the CTA exactly");
   extern __shared__ float4 g_smem[];
-  float4 *s_vis = g_smem;                  // [kVisBatch][2]: (re XX, re XY, re YX, re YY), (im ...)
-  float4 *s_t = s_vis + kVisBatch * 2;     // [kVisBatch][2]: (u, v, w, -), (bu, bv, bw, -)
-  float4 *s_lmn = s_t + kVisBatch * 2;     // [N*N]: (l, m, n', -) per pixel
+  float4 *s_vis = g_smem;                  // [vis_batch][2]: (re XX, re XY, re YX, re YY), (im ...)
+  float4 *s_t = s_vis + vis_batch * 2;     // [time_batch][2]: (u, v, w, -), (bu, bv, bw, -)
+  float4 *s_lmn = s_t + time_batch * 2;    // [N*N]: (l, m, n', -) per pixel
   float *s_kd = reinterpret_cast<float *>(s_lmn + N * N);   // [kMaxChan]
 
   const int tid = threadIdx.x;
@@ -114,13 +114,13 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
   int cur_slot = m.aterm_slot;
   bool flushed = false;
 
-  const int tb_max = n_chan >= kVisBatch ? 1 : kVisBatch / n_chan;  // timesteps per batch
+  const int tb_max = n_chan >= vis_batch ? 1 : min(vis_batch / n_chan, time_batch);  // timesteps per batch
   const float *uvw_b = uvw + (size_t)m.baseline * T * 3;
 
   for (int t0 = 0; t0 < n_time; t0 += tb_max) {
     const int tb = min(tb_max, n_time - t0);
-    for (int c_lo = 0; c_lo < n_chan; c_lo += kVisBatch) {   // only loops when n_chan > batch
-      const int nc = min(kVisBatch, n_chan - c_lo);
+    for (int c_lo = 0; c_lo < n_chan; c_lo += vis_batch) {   // only loops when n_chan > batch
+      const int nc = min(vis_batch, n_chan - c_lo);
       __syncthreads();
       // stage visibilities [tb][nc], re-packed into polarisation pairs, and the per-timestep terms
       for (int i = tid; i < tb * nc; i += NT) {
@@ -201,15 +201,21 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
   flush(cur_slot, flushed);
 }
 
-template <int N, int NT, int PPT, int MINB>
+// VB visibilities and TB timesteps are staged per batch.  Every batch costs the CTA two barriers, at which its
+// faster warps idle; larger batches measured +2.5 % (N = 32, 48) and up to +10 % (N = 24, blocks of 2048-4096
+// visibilities) over 256-visibility batches.  Single-channel plans keep 256 timesteps per batch.
+template <int N, int NT, int PPT, int MINB, int VB, int TB>
 static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
                     const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
-  constexpr size_t smem = sizeof(float4) * (kVisBatch * 4 + N * N) + sizeof(float) * kMaxChan;
   const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
   // single-channel plans without the span flag take the ONECHAN instance
   const bool one = !span && plan->max_n_chan == 1;
-  auto kern = span ? gridder_kernel<N, NT, PPT, MINB, true, false>
-                   : (one ? gridder_kernel<N, NT, PPT, MINB, false, true> : gridder_kernel<N, NT, PPT, MINB, false, false>);
+  constexpr size_t smem_one = sizeof(float4) * (256 * 4 + N * N) + sizeof(float) * kMaxChan;
+  constexpr size_t smem_any = sizeof(float4) * ((size_t)VB * 2 + (size_t)TB * 2 + N * N) + sizeof(float) * kMaxChan;
+  const size_t smem = one ? smem_one : smem_any;
+  auto kern = span ? gridder_kernel<N, NT, PPT, MINB, VB, TB, true, false>
+                   : (one ? gridder_kernel<N, NT, PPT, MINB, 256, 256, false, true>
+                          : gridder_kernel<N, NT, PPT, MINB, VB, TB, false, false>);
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(unsigned)np, NT, smem, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
@@ -224,10 +230,15 @@ int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, co
   if (np < 0) np = plan->P - p0;
   if (np <= 0) return IDG_OK;
   switch (plan->prm.subgrid_size) {
-    case 16: return launch_n<16, 64, 4, 8>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
-    case 24: return launch_n<24, 96, 6, 5>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
-    case 32: return launch_n<32, 256, 4, 2>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
-    case 48: return launch_n<48, 384, 6, 1>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 16: return launch_n<16, 64, 4, 8, 512, 128>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 24:
+      // 96-thread CTAs lose ~8 % once a block takes more than four batches (the three warps of a CTA drift apart
+      // between barriers); blocks that long go to 64 threads x 9 pixels, which does not show the effect
+      if (plan->P > 0 && plan->n_planned / plan->P > 4096)
+        return launch_n<24, 64, 9, 6, 512, 128>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+      return launch_n<24, 96, 6, 5, 1024, 64>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 32: return launch_n<32, 256, 4, 2, 512, 512>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 48: return launch_n<48, 384, 6, 1, 2048, 512>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 }
