@@ -115,6 +115,21 @@ static int finish_plan(idg_plan *pl, const double *freqs_host, cudaStream_t stre
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->freqs_dev, freqs_host, sizeof(double) * pl->C,
                                cudaMemcpyHostToDevice, stream));
   IDG_CUDA_TRY(cudaStreamSynchronize(stream));
+  {
+    // pixel direction cosines (R1: l_x = (x - N/2) S/N; R2: n' = sqrt(1 - l^2 - m^2) - 1 in its cancellation-free
+    // form), the same for every subgrid of the plan
+    std::vector<float4> lmn((size_t)N * N);
+    for (int32_t y = 0; y < N; ++y)
+      for (int32_t x = 0; x < N; ++x) {
+        const double l = (double)(x - N / 2) * pl->prm.image_size / (double)N;
+        const double m = (double)(y - N / 2) * pl->prm.image_size / (double)N;
+        const double r2 = l * l + m * m;
+        lmn[(size_t)y * N + x] = make_float4((float)l, (float)m, (float)(-r2 / (1.0 + std::sqrt(1.0 - r2))), 0.f);
+      }
+    IDG_CUDA_TRY(cudaMalloc(&pl->lmn_dev, sizeof(float4) * lmn.size()));
+    IDG_CUDA_TRY(cudaMemcpyAsync(pl->lmn_dev, lmn.data(), sizeof(float4) * lmn.size(), cudaMemcpyHostToDevice, stream));
+    IDG_CUDA_TRY(cudaStreamSynchronize(stream));
+  }
   if (pl->P > 0)
     IDG_CUDA_TRY(cudaMalloc(&pl->subgrids_dev, sizeof(float2) * 4 * N * N * (size_t)pl->P));
   return build_adder_lists(pl, stream);
@@ -142,7 +157,7 @@ int idg_last_cuda_error(void) { return g_last_cuda_error; }
 
 void idg_plan_destroy(idg_plan *pl) {
   if (!pl) return;
-  cudaFree(pl->meta_dev); cudaFree(pl->freqs_dev); cudaFree(pl->subgrids_dev);
+  cudaFree(pl->meta_dev); cudaFree(pl->freqs_dev); cudaFree(pl->lmn_dev); cudaFree(pl->subgrids_dev);
   cudaFree(pl->adder_list_dev); cudaFree(pl->adder_items_dev);
   cudaFree(pl->h_uvw_dev); cudaFree(pl->h_vis_dev); cudaFree(pl->h_aterms_dev);
   cudaFree(pl->h_grid_dev); cudaFree(pl->h_taper_dev);

@@ -33,6 +33,7 @@ struct idg_plan {
   std::vector<idg_subgrid_meta> meta_host;
   idg_subgrid_meta *meta_dev = nullptr;
   double *freqs_dev = nullptr;        // [C] Hz
+  float4 *lmn_dev = nullptr;          // [N*N] (l, m, n', 0) per subgrid pixel (R1, R2), rounded from FP64
   float2 *subgrids_dev = nullptr;     // [P][4][N][N]
   // adder: subgrids bucketed by the grid tiles they overlap (stable in p -> fixed order)
   int4 *adder_list_dev = nullptr;     // {subgrid index, x0 - tile_x, y0 - tile_y, 0}, grouped by tile

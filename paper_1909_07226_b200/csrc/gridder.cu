@@ -36,7 +36,7 @@ __device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); 
 template <int N, int NT, int PPT, int MINB, int VB, int TB, bool SPAN, bool ONECHAN>
 __global__ void __launch_bounds__(NT, MINB)
 gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
-               const double *__restrict__ freqs, const float4 *__restrict__ vis,
+               const double *__restrict__ freqs, const float4 *__restrict__ lmn, const float4 *__restrict__ vis,
                const float4 *__restrict__ aterms, const float *__restrict__ taper,
                float2 *__restrict__ subgrids, int32_t T, int32_t C, int32_t n_stations,
                int32_t L, double image_size, double w_step, int32_t aterm_interval) {
@@ -61,17 +61,10 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
   for (int c = tid; c < n_chan; c += NT)
     s_kd[c] = (float)(two_pi * (freqs[m.chan_begin + c] * inv_c0 - k_mid));
 
-  // pixel direction cosines (R1: l_x = (x - N/2) S/N; R2: n' = sqrt(1-l^2-m^2) - 1), kept in
-  // shared memory: they are needed once per timestep only, not in the channel loop
+  // pixel direction cosines (l, m, n') from the plan's table, kept in shared memory: they are needed once per
+  // timestep only, not in the channel loop
 #pragma unroll
-  for (int k = 0; k < PPT; ++k) {
-    const int pix = tid + k * NT;
-    const int y = pix / N, x = pix - y * N;
-    const double l = (double)(x - N / 2) * image_size / (double)N;
-    const double mm = (double)(y - N / 2) * image_size / (double)N;
-    const double r2 = l * l + mm * mm;
-    s_lmn[pix] = make_float4((float)l, (float)mm, (float)(-r2 / (1.0 + sqrt(1.0 - r2))), 0.f);
-  }
+  for (int k = 0; k < PPT; ++k) s_lmn[tid + k * NT] = __ldg(&lmn[tid + k * NT]);
 
   float2 re01[PPT], re23[PPT], im01[PPT], im23[PPT];
 #pragma unroll
@@ -218,7 +211,7 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, c
                           : gridder_kernel<N, NT, PPT, MINB, VB, TB, false, false>);
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<(unsigned)np, NT, smem, stream>>>(
-      plan->meta_dev + p0, uvw, plan->freqs_dev, reinterpret_cast<const float4 *>(vis),
+      plan->meta_dev + p0, uvw, plan->freqs_dev, plan->lmn_dev, reinterpret_cast<const float4 *>(vis),
       reinterpret_cast<const float4 *>(aterms), taper, subgrids + (size_t)p0 * 4 * N * N, plan->T, plan->C,
       plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
   IDG_CUDA_TRY(cudaGetLastError());
