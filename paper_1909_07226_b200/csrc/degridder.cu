@@ -215,11 +215,16 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
   // more channels per thread amortise the per-pixel shared-memory reads and phase set-up, as long as the
   // largest block still fills a 128-thread CTA
   int cpt = mc >= 4 ? 4 : (mc >= 2 ? 2 : 1);
-  if (mc >= 8 && plan->max_n_time * ((mc + 7) / 8) >= 128) cpt = 8;
+  const int items8 = plan->max_n_time * ((mc + 7) / 8);
+  // 8 channels per thread when that still fills a 128-thread CTA, or (N >= 32) half of one: then two thread groups
+  // share the pixels (SPLIT below)
+  if (mc >= 8 && (items8 >= 128 || (N >= 32 && items8 >= 32 && items8 <= 64))) cpt = 8;
   // plans that mix channel-group sizes (a 20-channel band cut into 16 + 4): do not idle more than 5 % of the slots
   while (cpt > 1 && plan->dg_waste[cpt == 8 ? 3 : (cpt == 4 ? 2 : 1)] > 0.05f) cpt /= 2;
   const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
   const bool small = items <= 128;
+  if (N >= 32 && items <= 64 && cpt == 8)
+    return launch_k<(N >= 32 ? N : 32), 128, 8, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
   if (items <= 64 && cpt <= 4 && N >= 24) {   // short blocks: split the pixels over thread groups (measured: no gain at N = 16)
     if (cpt == 4) return launch_k<N, 128, 4, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     if (cpt == 2) return launch_k<N, 128, 2, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
