@@ -403,7 +403,11 @@ def test_ska_slice_sampled():
 # BASELINE.json configs[4]: corners of the kernel sweep (forced blocks), sampled against the oracle
 # ---------------------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("N,max_c,max_t,a_int", [(16, 1, 32, 8), (32, 1, 64, 16), (24, 4, 64, 32), (32, 16, 512, 64), (48, 64, 512, 256)])
+@pytest.mark.parametrize("N,max_c,max_t,a_int", [(16, 1, 32, 8), (32, 1, 64, 16), (24, 4, 64, 32), (32, 16, 512, 64), (48, 64, 512, 256),
+                                                 # long blocks: many staging batches per CTA; N = 24 above 4096 visibilities per
+                                                 # block takes the 64-thread gridder instance; (32, 16, 512, 32) the degridder
+                                                 # with 8 channels per thread and two pixel groups
+                                                 (16, 64, 512, 128), (24, 16, 256, 256), (24, 16, 512, 512), (32, 16, 512, 32)])
 def test_sweep_corners_sampled(N, max_c, max_t, a_int):
     w = synth.make_workload("sweep", n_baselines=12, n_time=512, subgrid_size=N, max_channels=max_c,
                             max_timesteps=max_t, aterm_interval=a_int)
