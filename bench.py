@@ -36,7 +36,7 @@ LANE_OPS_PER_VIS_PIXEL = 18
 ALU_PEAK_TFLOPS = N_SM * FP32_LANES * 2 * SM_MAX_HZ / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of one gridder launch from the committed ncu --set full capture
 # (profiles/r01_final_ncu_summary.md); only the workload that was captured has a number
-NCU_TRAFFIC_BYTES = {"lofar": 159004416 + 108203776}
+NCU_TRAFFIC_BYTES = {"lofar": 159668480 + 108218624}
 
 
 def parse_args():
