@@ -95,11 +95,12 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
       // stage Dg = A1 (taper Ip) A2^H and the pixel coordinates for this chunk
       for (int i = tid; i < npx; i += NT) {
         const int pix = pix0 + i;
-        if (CPT >= 8) {
+        if (CPT >= 8 && !(N == 16 && NT == 256)) {
           s_lmn[i] = __ldg(&lmn[pix]);       // the plan's table
         } else {
-          // measured: with 1-4 channels per thread the kernel is 2 % faster when the staging phase computes the
-          // direction cosines (same values as the table: R1, R2 in FP64, rounded once) instead of loading them
+          // measured: with 1-4 channels per thread (and in the N = 16, 256-thread instance) the kernel is 2-4 % faster
+          // when the staging phase computes the direction cosines (same values as the table: R1, R2 in FP64,
+          // rounded once) instead of loading them
           const int y = pix / N, x = pix - y * N;
           const double l = (double)(x - N / 2) * image_size / (double)N;
           const double mm = (double)(y - N / 2) * image_size / (double)N;
