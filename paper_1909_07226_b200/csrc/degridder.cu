@@ -20,7 +20,9 @@ __device__ __forceinline__ float2 dbc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 dlo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 dhi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int CPT, bool SPAN, bool SPLIT, bool ONECHAN = false>
+// FILT selects the subgrids a launch works on (plans that mix channel-group sizes are degridded in two launches):
+// 0 all, 1 only those with n_chan a multiple of 8, 2 only the others.
+template <int N, int NT, int CPT, bool SPAN, bool SPLIT, bool ONECHAN = false, int FILT = 0>
 __global__ void __launch_bounds__(NT, NT == 128 ? 4 : 2)
 degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                  const double *__restrict__ freqs, const float4 *__restrict__ lmn,
@@ -42,6 +44,8 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
   const int tid = threadIdx.x;
   const idg_subgrid_meta m = meta[blockIdx.x];
   const int n_chan = m.n_chan, n_time = m.n_time;
+  if (FILT == 1 && (n_chan & 7) != 0) return;
+  if (FILT == 2 && (n_chan & 7) == 0) return;
   const double two_pi = 6.283185307179586476925286766559;
   const double inv_c0 = 1.0 / kSpeedOfLight;
   const double u0 = (double)(m.x0 + N / 2 - L / 2) / image_size;
@@ -207,6 +211,21 @@ static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgri
   return IDG_OK;
 }
 
+// one of the two launches of a plan that mixes channel-group sizes (FILT 1: 8 channels per thread on the subgrids
+// whose channel count is a multiple of 8; FILT 2: 4 per thread on the rest)
+template <int N, int NT, int CPT, int FILT>
+static int launch_filtered(const idg_plan *plan, const float *uvw, const float2 *subgrids,
+                           const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
+                           int64_t p0, int64_t np) {
+  degridder_kernel<N, NT, CPT, false, false, false, FILT><<<(unsigned)np, NT, 0, stream>>>(
+      plan->meta_dev + p0, uvw, plan->freqs_dev, plan->lmn_dev, subgrids + (size_t)p0 * 4 * N * N,
+      reinterpret_cast<const float4 *>(aterms),
+      taper, reinterpret_cast<float4 *>(vis_out), plan->T, plan->C, plan->n_stations,
+      plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
+  IDG_CUDA_TRY(cudaGetLastError());
+  return IDG_OK;
+}
+
 template <int N>
 static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgrids,
                     const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
@@ -220,7 +239,18 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
   // 8 channels per thread when that still fills a 128-thread CTA, or (N >= 32) half of one: then two thread groups
   // share the pixels (SPLIT below)
   if (mc >= 8 && (items8 >= 128 || (N >= 32 && items8 >= 32 && items8 <= 64))) cpt = 8;
-  // plans that mix channel-group sizes (a 20-channel band cut into 16 + 4): do not idle more than 5 % of the slots
+  // plans that mix channel-group sizes (a 20-channel band cut into 16 + 4) and would idle more than 5 % of the
+  // 8-channel slots: two launches, 8 channels per thread on the subgrids that fill them, 4 on the rest
+  if (cpt == 8 && items8 >= 128 && plan->dg_waste[3] > 0.05f && plan->dg_waste[2] <= 0.05f &&
+      (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) == 0) {
+    int rc = items8 <= 128 ? launch_filtered<N, 128, 8, 1>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np)
+                           : launch_filtered<N, 256, 8, 1>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    if (rc != IDG_OK) return rc;
+    return plan->max_n_time <= 128
+               ? launch_filtered<N, 128, 4, 2>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np)
+               : launch_filtered<N, 256, 4, 2>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+  }
+  // otherwise: do not idle more than 5 % of the slots
   while (cpt > 1 && plan->dg_waste[cpt == 8 ? 3 : (cpt == 4 ? 2 : 1)] > 0.05f) cpt /= 2;
   const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
   const bool small = items <= 128;

@@ -416,6 +416,16 @@ def test_sweep_corners_sampled(N, max_c, max_t, a_int):
     assert P == 12 * (512 // eff_t) * (64 // max_c)
 
 
+def test_mixed_channel_groups_paper_shape_sampled():
+    """A slice of the paper-shaped workload (20 channels cut into groups of 16 + 4, N = 48): the degridder runs as two
+    launches, 8 channels per thread on the 16-channel subgrids and 4 per thread on the 4-channel ones."""
+    w = synth.make_workload("paper", n_baselines=10, n_time=512, baseline_offset=700)
+    _, _, meta = _plan_both(w)
+    assert set(np.unique(meta["n_chan"]).tolist()) >= {4, 16}
+    assert int(meta["n_time"].max()) * 2 >= 128          # the condition for 8 channels per thread
+    assert _sampled_full_size_check(w, 12, 77) == len(meta)
+
+
 # ---------------------------------------------------------------------------------------------
 # NEXT-1: image-plane wrap with W-stacking (paper_1909_07226_b200.imaging) against the oracle
 # ---------------------------------------------------------------------------------------------
