@@ -245,10 +245,12 @@ def run_b200(args):
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(args.steps)]
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    launches0 = idg.idg_kernel_launches()
     start.record(stream)
     for k in range(args.steps):
         step(evs[k])
     stop.record(stream)
+    gpu_launches = idg.idg_kernel_launches() - launches0      # counted by the library at its launch sites
     torch.cuda.synchronize()
     clocks = sampler.stop()
     if world > 1:
@@ -353,7 +355,7 @@ def run_b200(args):
         "config": {"workload": WORKLOAD_NAMES[args.workload], "subgrid_size": N, "grid_size": L,
                    "parallelism": "baselines sharded, %d replica(s), no collective" % world,
                    "l2": "inputs larger than L2 (vis + subgrids + grid > 126 MB)" if args.workload != "tiny" else "fits L2"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": 6 * args.steps, "roofline": roofline, "detail": extra,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": gpu_launches, "roofline": roofline, "detail": extra,
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(w.to("cpu"))

@@ -76,6 +76,9 @@ typedef struct idg_plan idg_plan; /* opaque; owns metadata (host + device), adde
 
 const char *idg_strerror(int code);
 int idg_last_cuda_error(void);
+/* Number of CUDA kernels this library has launched in the process so far (all entry points, all threads);
+ * the difference of two readings counts the launches in between.  Host-side bookkeeping only, never fails. */
+long long idg_kernel_launches(void);
 
 /* ---- planner (a0): section 3.2, Fig. 2; readings R10-R12 -----
  * Partitions every baseline's (time x channel) samples into blocks whose uv extent in grid

@@ -22,7 +22,7 @@ META_DTYPE = np.dtype([(n, "<i4") for n in (
 assert META_DTYPE.itemsize == 48
 
 EXPORTS = (
-    "idg_strerror", "idg_last_cuda_error", "idg_plan_create", "idg_plan_from_metadata",
+    "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_plan_create", "idg_plan_from_metadata",
     "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
     "idg_adder", "idg_splitter", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
@@ -54,6 +54,8 @@ def lib() -> ctypes.CDLL:
                            "(needs nvcc); there is no CPU fallback")
         _lib = ctypes.CDLL(LIB_PATH)
         _lib.idg_strerror.restype = ctypes.c_char_p
+        _lib.idg_kernel_launches.restype = ctypes.c_longlong
+        _lib.idg_kernel_launches.argtypes = []
         _lib.idg_strerror.argtypes = [ctypes.c_int]
         _lib.idg_plan_destroy.restype = None
         _lib.idg_plan_destroy.argtypes = [ctypes.c_void_p]
@@ -169,6 +171,11 @@ class _DevView:
         self._owner = owner
         self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": "<f4", "data": (int(ptr), False),
                                          "version": 2, "strides": None}
+
+
+def idg_kernel_launches() -> int:
+    """Kernels launched by the library in this process so far (host-side counter)."""
+    return int(lib().idg_kernel_launches())
 
 
 def idg_plan_create(params, uvw: torch.Tensor, freqs, baselines, n_stations: int, stream=None) -> Plan:

@@ -119,7 +119,7 @@ int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cud
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 #undef IDG_ADD
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 
@@ -141,7 +141,7 @@ int launch_splitter(const idg_plan *plan, const float2 *grid, float2 *subgrids,
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 #undef IDG_SPL
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 

@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/idg_b200.h: argument checks, plan ownership, stage sequencing.
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstring>
 #include <new>
@@ -10,6 +11,8 @@ namespace idg {
 
 static thread_local int g_last_cuda_error = 0;
 void set_last_cuda_error(cudaError_t e) { g_last_cuda_error = (int)e; }
+static std::atomic<long long> g_kernel_launches{0};
+void count_launch() { g_kernel_launches.fetch_add(1, std::memory_order_relaxed); }
 
 static bool supported_size(int n) { return n == 16 || n == 24 || n == 32 || n == 48; }
 static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
@@ -154,6 +157,8 @@ const char *idg_strerror(int code) {
 }
 
 int idg_last_cuda_error(void) { return g_last_cuda_error; }
+
+long long idg_kernel_launches(void) { return idg::g_kernel_launches.load(std::memory_order_relaxed); }
 
 void idg_plan_destroy(idg_plan *pl) {
   if (!pl) return;

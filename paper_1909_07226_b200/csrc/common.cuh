@@ -64,6 +64,15 @@ void set_last_cuda_error(cudaError_t e);
     }                                                        \
   } while (0)
 
+// kernels launched by this library since it was loaded (idg_kernel_launches); every launch site checks with
+// IDG_LAUNCH_CHECK, which counts it
+void count_launch();
+#define IDG_LAUNCH_CHECK()             \
+  do {                                 \
+    idg::count_launch();               \
+    IDG_CUDA_TRY(cudaGetLastError()); \
+  } while (0)
+
 // planner (plan.cu)
 int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *freqs_host,
                 const int32_t *baselines_host, int32_t B, int32_t T, int32_t C,

@@ -207,7 +207,7 @@ static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgri
       reinterpret_cast<const float4 *>(aterms),
       taper, reinterpret_cast<float4 *>(vis_out), plan->T, plan->C, plan->n_stations,
       plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 
@@ -222,7 +222,7 @@ static int launch_filtered(const idg_plan *plan, const float *uvw, const float2 
       reinterpret_cast<const float4 *>(aterms),
       taper, reinterpret_cast<float4 *>(vis_out), plan->T, plan->C, plan->n_stations,
       plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 

@@ -226,7 +226,7 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, c
       plan->meta_dev + p0, uvw, plan->freqs_dev, plan->lmn_dev, reinterpret_cast<const float4 *>(vis),
       reinterpret_cast<const float4 *>(aterms), taper, subgrids + (size_t)p0 * 4 * N * N, plan->T, plan->C,
       plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 

@@ -70,7 +70,7 @@ int idg_image_w_accumulate(void *acc_dev, const void *layer_dev, int32_t L, doub
   const dim3 grid((L + 63) / 64, (L + 3) / 4);
   image_w_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>((float2 *)acc_dev, (const float2 *)layer_dev, L,
                                                               image_size, w0, (double)sign);
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 
@@ -80,7 +80,7 @@ int idg_image_w_apply(void *out_dev, const void *in_dev, int32_t L, double image
   const dim3 grid((L + 63) / 64, (L + 3) / 4);
   image_w_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>((float2 *)out_dev, (const float2 *)in_dev, L,
                                                                image_size, w0, (double)sign);
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 
@@ -88,7 +88,7 @@ int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *st
   if (!image_dev || !cbar_dev || L < 1) return IDG_ERR_INVALID_ARG;
   const dim3 grid((L + 63) / 64, (L + 3) / 4);
   image_divide_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((float2 *)image_dev, cbar_dev, L);
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 

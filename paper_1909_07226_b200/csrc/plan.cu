@@ -165,6 +165,7 @@ int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *
   const int blocks = (B + threads - 1) / threads;
   plan_kernel<false><<<blocks, threads, 0, stream>>>(pc, uvw_dev, freqs_dev, scale_dev, bl_dev,
                                                      counts_dev, nullptr, nullptr);
+  count_launch();
   PLAN_TRY(cudaGetLastError());
   std::vector<int64_t> counts(3 * (size_t)B);
   PLAN_TRY(cudaMemcpyAsync(counts.data(), counts_dev, sizeof(int64_t) * 3 * (size_t)B,
@@ -182,6 +183,7 @@ int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *
                              cudaMemcpyHostToDevice, stream));
     plan_kernel<true><<<blocks, threads, 0, stream>>>(pc, uvw_dev, freqs_dev, scale_dev, bl_dev,
                                                       nullptr, offsets_dev, meta_dev);
+    count_launch();
     PLAN_TRY(cudaGetLastError());
     PLAN_TRY(cudaMemcpyAsync(meta_out.data(), meta_dev, sizeof(idg_subgrid_meta) * (size_t)P,
                              cudaMemcpyDeviceToHost, stream));

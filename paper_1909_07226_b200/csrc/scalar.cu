@@ -260,7 +260,7 @@ static int launch_gs(const idg_plan *plan, const float *uvw, const float2 *vis, 
     gridder_scalar_kernel<N, NT, PPT, MINB, 1><<<(unsigned)plan->P, NT, 0, stream>>>(
         plan->meta_dev, uvw, plan->freqs_dev, vis, gains, taper, subgrids, plan->T, plan->C, plan->n_stations,
         plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, 0.f);
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 
@@ -289,7 +289,7 @@ static int launch_ds(const idg_plan *plan, const float *uvw, const float2 *subgr
   if (cpt == 8 && dkd != 0.f) IDG_DS(8, 4); else if (cpt == 4 && dkd != 0.f) IDG_DS(4, 4);
   else if (cpt == 8) IDG_DS(8, 1); else if (cpt == 4) IDG_DS(4, 1); else if (cpt == 2) IDG_DS(2, 1); else IDG_DS(1, 1);
 #undef IDG_DS
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 

@@ -81,7 +81,7 @@ static int launch_n(const idg_plan *plan, float2 *subgrids, int direction, cudaS
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     subgrid_fft_kernel<N, true><<<(unsigned)np, 4 * N, smem, stream>>>(subgrids);
   }
-  IDG_CUDA_TRY(cudaGetLastError());
+  IDG_LAUNCH_CHECK();
   return IDG_OK;
 }
 

@@ -86,6 +86,31 @@ def tiny_case():
     return dict(w=w, wc=wc, prm=prm, plan=plan, meta=meta, d=_np(w))
 
 
+def test_kernel_launch_counter(tiny_case):
+    """idg_kernel_launches (what bench.py reports as gpu_launches) counts one per stage call, three / three for
+    idg_grid / idg_degrid."""
+    c = tiny_case
+    wc, plan = c["wc"], c["plan"]
+    L = c["prm"].grid_size
+    sub = plan.subgrids()
+    grid = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    out = torch.zeros_like(wc.vis)
+    n0 = idg.idg_kernel_launches()
+    idg.idg_gridder(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, sub)
+    assert idg.idg_kernel_launches() - n0 == 1
+    idg.idg_subgrid_fft(plan, sub, -1)
+    idg.idg_adder(plan, sub, grid)
+    idg.idg_splitter(plan, grid, sub)
+    idg.idg_subgrid_fft(plan, sub, +1)
+    idg.idg_degridder(plan, wc.uvw, sub, wc.aterms, wc.taper, out)
+    assert idg.idg_kernel_launches() - n0 == 6
+    idg.idg_grid(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, grid)
+    assert idg.idg_kernel_launches() - n0 == 9
+    idg.idg_degrid(plan, wc.uvw, grid, wc.aterms, wc.taper, out)
+    assert idg.idg_kernel_launches() - n0 == 12
+    torch.cuda.synchronize()
+
+
 def test_gridder_stage(tiny_case):
     c = tiny_case
     ref = orc.gridder(c["prm"], c["meta"], c["d"]["uvw"], c["d"]["freqs"], c["d"]["vis"], c["d"]["aterms"], c["d"]["taper"])
