@@ -143,6 +143,11 @@ int idg_adder(const idg_plan *plan, const void *subgrids_dev, void *grid_dev, vo
 /* a4 splitter: V_p[pol][b][a] = grid[pol][y0+b][x0+a]. */
 int idg_splitter(const idg_plan *plan, const void *grid_dev, void *subgrids_dev,
                  void *cuda_stream);
+/* a4 + a5 in one kernel (what idg_degrid runs): the inverse subgrid FFT gathers its input from the grid window
+ * instead of reading the splitter's copy, I_p = IFFT(V[pol][y0..y0+N)[x0..x0+N)).  Bit-identical
+ * to idg_splitter followed by idg_subgrid_fft(+1); subgrids_dev [P][4][N][N] is written, grid_dev only read. */
+int idg_splitter_ifft(const idg_plan *plan, const void *grid_dev, void *subgrids_dev,
+                      void *cuda_stream);
 /* a6 degridder: Alg. 2: Dg = A1 (taper Ip) A2^H per pixel, then
  *   Y_k = sum_xy Dg[y][x] exp(-2 pi i (du l_x + dv m_y + dw n'_xy)) -> vis_out (planned only). */
 int idg_degridder(const idg_plan *plan, const float *uvw_dev, const void *subgrids_dev,

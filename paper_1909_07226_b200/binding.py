@@ -25,7 +25,7 @@ EXPORTS = (
     "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_plan_create", "idg_plan_from_metadata",
     "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
-    "idg_adder", "idg_splitter", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
+    "idg_adder", "idg_splitter", "idg_splitter_ifft", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
     "idg_image_divide", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
 
 
@@ -270,6 +270,13 @@ def idg_splitter(plan: Plan, grid, subgrids, stream=None) -> None:
     _shape_check(plan, subgrids=subgrids, grid=grid)
     _check(lib().idg_splitter(plan.handle, _dev(grid, _C64, "grid"), _dev(subgrids, _C64, "subgrids"),
                               _stream(stream)), "idg_splitter")
+
+
+def idg_splitter_ifft(plan: Plan, grid, subgrids, stream=None) -> None:
+    """Rows a4 + a5 in one kernel: subgrids = IFFT of the grid windows."""
+    _shape_check(plan, subgrids=subgrids, grid=grid)
+    _check(lib().idg_splitter_ifft(plan.handle, _dev(grid, _C64, "grid"), _dev(subgrids, _C64, "subgrids"),
+                              _stream(stream)), "idg_splitter_ifft")
 
 
 def idg_degridder(plan: Plan, uvw, subgrids, aterms, taper, vis_out, stream=None) -> None:

@@ -107,6 +107,11 @@ int idg_splitter(const idg_plan *pl, const void *grid_dev, void *subgrids_dev, v
   return launch_splitter(pl, (const float2 *)grid_dev, (float2 *)subgrids_dev, S(stream));
 }
 
+int idg_splitter_ifft(const idg_plan *pl, const void *grid_dev, void *subgrids_dev, void *stream) {
+  if (!pl || (!subgrids_dev && pl->P > 0) || !grid_dev) return IDG_ERR_INVALID_ARG;
+  return launch_splitter_ifft(pl, (const float2 *)grid_dev, (float2 *)subgrids_dev, S(stream));
+}
+
 int idg_degridder(const idg_plan *pl, const float *uvw_dev, const void *subgrids_dev,
                   const void *aterms_dev, const float *taper_dev, void *vis_out_dev, void *stream) {
   if (!pl || !uvw_dev || (!subgrids_dev && pl->P > 0) || !aterms_dev || !taper_dev || !vis_out_dev)
@@ -130,8 +135,7 @@ int idg_degrid(const idg_plan *pl, const float *uvw_dev, const void *grid_dev,
   if (!pl || !uvw_dev || !grid_dev || !aterms_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
   if (pl->n_skipped > 0)  // skipped samples read as 0; planned ones are overwritten below
     IDG_CUDA_TRY(cudaMemsetAsync(vis_out_dev, 0, sizeof(float2) * 4 * (size_t)pl->B * pl->T * pl->C, S(stream)));
-  int rc = launch_splitter(pl, (const float2 *)grid_dev, pl->subgrids_dev, S(stream));
-  if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, +1, S(stream));
+  int rc = launch_splitter_ifft(pl, (const float2 *)grid_dev, pl->subgrids_dev, S(stream));
   if (rc == IDG_OK)
     rc = launch_degridder(pl, uvw_dev, pl->subgrids_dev, (const float2 *)aterms_dev, taper_dev,
                           (float2 *)vis_out_dev, S(stream));
@@ -249,8 +253,7 @@ int idg_degrid_host(idg_plan *pl, const float *uvw_host, const void *grid_host,
     IDG_CUDA_TRY(cudaMemsetAsync(pl->h_vis_dev, 0, sizeof(float2) * 4 * nvis, s));
   for (size_t k = 0; k < chunks.size(); ++k) {
     const HostChunk &ch = chunks[k];
-    rc = launch_splitter(pl, pl->h_grid_dev, pl->subgrids_dev, s, ch.p0, ch.p1 - ch.p0);
-    if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, +1, s, ch.p0, ch.p1 - ch.p0);
+    rc = launch_splitter_ifft(pl, pl->h_grid_dev, pl->subgrids_dev, s, ch.p0, ch.p1 - ch.p0);
     if (rc == IDG_OK)
       rc = launch_degridder(pl, pl->h_uvw_dev, pl->subgrids_dev, pl->h_aterms_dev, pl->h_taper_dev, pl->h_vis_dev, s,
                             ch.p0, ch.p1 - ch.p0);

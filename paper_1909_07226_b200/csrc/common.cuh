@@ -90,6 +90,8 @@ int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgr
 int launch_subgrid_fft(const idg_plan *plan, float2 *subgrids, int direction, cudaStream_t stream,
                        int64_t p0 = 0, int64_t np = -1);
 int launch_adder(const idg_plan *plan, const float2 *subgrids, float2 *grid, cudaStream_t stream, int n_pol = 4);
+int launch_splitter_ifft(const idg_plan *plan, const float2 *grid, float2 *subgrids, cudaStream_t stream,
+                         int64_t p0 = 0, int64_t np = -1);
 int launch_splitter(const idg_plan *plan, const float2 *grid, float2 *subgrids,
                     cudaStream_t stream, int64_t p0 = 0, int64_t np = -1, int n_pol = 4);
 // scalar variant (NEXT-3, scalar.cu): vis [B][T][C], gains [slots][stations][N][N], subgrids [P][N][N]
