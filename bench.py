@@ -2,8 +2,8 @@
 """bench.py -- throughput of the IDG hot path on B200 (driver contract, tier-specific reading).
 
 One "step" = one pass of the whole hot path over one synthetic workload that is resident in HBM:
-Alg. 1 (gridder -> subgrid FFT -> adder) followed by Alg. 2 (splitter -> subgrid IFFT ->
-degridder) with a plan made beforehand (the partition is an INPUT of both algorithms,
+Alg. 1 (gridder -> subgrid FFT -> adder) followed by Alg. 2 (splitter + subgrid IFFT, one fused
+kernel -> degridder) with a plan made beforehand (the partition is an INPUT of both algorithms,
 PAPER.md:276 / PAPER.md:315; the planner is timed separately and reported as plan_ms).
 value = (visibilities gridded + visibilities degridded) / time, in MVis/s, over all ranks.
 
