@@ -449,6 +449,21 @@ def test_sweep_corners_sampled(N, max_c, max_t, a_int):
     assert P == 12 * (512 // eff_t) * (64 // max_c)
 
 
+@pytest.mark.parametrize("N", [16, 32])
+def test_maximum_channels_per_subgrid(N):
+    """256 channels in one subgrid (the ABI's maximum): the gridder stages two timesteps per batch (N = 32, 16) and the
+    degridder runs 32 channel groups of 8 per timestep."""
+    w = synth.make_workload("tiny", subgrid_size=N, max_channels=256, max_timesteps=16)
+    rng = np.random.default_rng(256 + N)
+    freqs = 150e6 + 10e3 * np.arange(256, dtype=np.float64)
+    vis = torch.from_numpy((rng.standard_normal((w.B, w.T, 256, 4)) + 1j * rng.standard_normal((w.B, w.T, 256, 4)))
+                           .astype(np.complex64))
+    w = dataclasses.replace(w, freqs=freqs, vis=vis)
+    _, _, meta = _plan_both(w)
+    assert int(meta["n_chan"].max()) == 256
+    _sampled_full_size_check(w, 8, 300 + N)
+
+
 def test_mixed_channel_groups_paper_shape_sampled():
     """A slice of the paper-shaped workload (20 channels cut into groups of 16 + 4, N = 48): the degridder runs as two
     launches, 8 channels per thread on the 16-channel subgrids and 4 per thread on the 4-channel ones."""
