@@ -74,6 +74,16 @@ typedef struct {
 typedef struct idg_plan idg_plan; /* opaque; owns metadata (host + device), adder work lists,
                                      the [P][4][N][N] subgrid scratch buffer and staging buffers */
 
+/* Re-entrancy: idg_grid, idg_degrid, the *_scalar and the *_host calls WRITE the plan-owned subgrid scratch
+ * (and the *_host calls the plan's staging buffers, copy stream and events) although the compute calls take a
+ * `const idg_plan *`: two such calls on ONE plan must be ordered on one stream (or by events); concurrent calls on
+ * one plan from two streams or two threads race.  Calls on different plans are independent.  The stage entry
+ * points touch only the buffers they are given.
+ * Alignment: vis, aterms, subgrids and vis_out are read / written as 16-byte vectors and must be 16-byte aligned
+ * (IDG_ERR_INVALID_ARG otherwise); grid, uvw and taper need only the alignment of their element type.
+ * A-term slots: every compute call takes n_slots, the first extent of the aterms (gains) array it is given; a plan
+ * that indexes a slot >= n_slots is refused with IDG_ERR_PLAN_MISMATCH before anything is launched. */
+
 const char *idg_strerror(int code);
 int idg_last_cuda_error(void);
 /* Number of CUDA kernels this library has launched in the process so far (all entry points, all threads);
@@ -105,16 +115,21 @@ int idg_plan_size(const idg_plan *plan, int64_t *n_subgrids, int64_t *n_planned_
 int idg_plan_metadata(const idg_plan *plan, idg_subgrid_meta *out_host, int64_t capacity);
 /* Device pointer of the plan-owned [P][4][N][N] complex64 scratch (valid until destroy). */
 int idg_plan_subgrids(const idg_plan *plan, void **subgrids_dev);
+/* Number of A-term slots the plan indexes: max over subgrids of the last slot + 1 (with IDG_PLAN_SPAN_ATERMS the
+ * slot of a block's last timestep decides); 0 for an empty plan. */
+int idg_plan_aterm_slots(const idg_plan *plan, int32_t *n_slots);
+/* w offset of a w layer, w0 = (w_index + 0.5) w_step, or 0 when w_step = 0 (Alg. 1, R4). */
+int idg_plan_w_offset(const idg_plan *plan, int32_t w_index, double *w0);
 void idg_plan_destroy(idg_plan *plan);
 
 /* ---- Algorithm 1 without its last line: gridder -> subgrid FFT -> adder.
  * ACCUMULATES into grid_dev (Alg. 1 zeroes V once; zeroing is the caller's). */
 int idg_grid(const idg_plan *plan, const float *uvw_dev, const void *vis_dev,
-             const void *aterms_dev, const float *taper_dev, void *grid_dev, void *cuda_stream);
+             const void *aterms_dev, int32_t n_slots, const float *taper_dev, void *grid_dev, void *cuda_stream);
 /* ---- Algorithm 2 after its first two lines: splitter -> subgrid IFFT ->
  * degridder.  Overwrites every planned visibility; skipped ones are set to 0. */
 int idg_degrid(const idg_plan *plan, const float *uvw_dev, const void *grid_dev,
-               const void *aterms_dev, const float *taper_dev, void *vis_out_dev,
+               const void *aterms_dev, int32_t n_slots, const float *taper_dev, void *vis_out_dev,
                void *cuda_stream);
 
 /* ---- the same two calls on HOST buffers (pinned or pageable): copy in, run, copy out,
@@ -132,7 +147,7 @@ int idg_degrid_host(idg_plan *plan, const float *uvw_host, const void *grid_host
  * a1 gridder: Eq. 25, Alg. 1, section 3.4 PAPER.md:247-249:
  *   Sg[y][x] = taper A1^H (sum_k Y_k exp(+2 pi i (du l_x + dv m_y + dw n'_xy))) A2  -> subgrids */
 int idg_gridder(const idg_plan *plan, const float *uvw_dev, const void *vis_dev,
-                const void *aterms_dev, const float *taper_dev, void *subgrids_dev,
+                const void *aterms_dev, int32_t n_slots, const float *taper_dev, void *subgrids_dev,
                 void *cuda_stream);
 /* a2 / a5 subgrid FFT: centred 2-D DFT of every plane in place, scale 1/N^2 both ways (R6);
  * direction -1 = forward exp(-..), +1 = inverse. */
@@ -151,7 +166,7 @@ int idg_splitter_ifft(const idg_plan *plan, const void *grid_dev, void *subgrids
 /* a6 degridder: Alg. 2: Dg = A1 (taper Ip) A2^H per pixel, then
  *   Y_k = sum_xy Dg[y][x] exp(-2 pi i (du l_x + dv m_y + dw n'_xy)) -> vis_out (planned only). */
 int idg_degridder(const idg_plan *plan, const float *uvw_dev, const void *subgrids_dev,
-                  const void *aterms_dev, const float *taper_dev, void *vis_out_dev,
+                  const void *aterms_dev, int32_t n_slots, const float *taper_dev, void *vis_out_dev,
                   void *cuda_stream);
 
 /* ---- image-plane side of W-stacking (OUTSIDE the timed hot path) --------------
@@ -163,12 +178,20 @@ int idg_degridder(const idg_plan *plan, const float *uvw_dev, const void *subgri
  *   idg_image_w_accumulate: acc += layer * exp(sign 2 pi i w0 n')
  *   idg_image_w_apply:      out  = in    * exp(sign 2 pi i w0 n')   (out may alias in)
  *   idg_image_divide:       image[pol][y][x] /= cbar[y][x], cbar [L][L] float32 (the image-domain taper c-bar)
+ *   idg_image_taper:        c-bar itself from the subgrid taper (below)
  * Errors: IDG_ERR_INVALID_ARG, IDG_ERR_CUDA. */
 int idg_image_w_accumulate(void *acc_dev, const void *layer_dev, int32_t L, double image_size, double w0,
                            int32_t sign, void *cuda_stream);
 int idg_image_w_apply(void *out_dev, const void *in_dev, int32_t L, double image_size, double w0, int32_t sign,
                       void *cuda_stream);
 int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *cuda_stream);
+/* c-bar, the image-domain taper that Alg. 1's last line divides by ("rms image domain kernel",
+ * PAPER.md:278): the [N][N] subgrid taper carried to the L x L image raster by the interpolation the method itself
+ * performs, section 4.2 ("the effective window is a sinc interpolation of the discrete window"): the
+ * periodic (Dirichlet-kernel) interpolation of the N samples at l_i = (i - N/2) S/N onto l_x = (x - L/2) S/L, both
+ * axes, real part.  FP64 arithmetic, float32 result.  taper_dev [N][N] float32, cbar_dev [L][L] float32, N in
+ * {16, 24, 32, 48}, L >= N even.  Asynchronous on cuda_stream; allocates (and frees, stream-ordered) 32 L N bytes. */
+int idg_image_taper(const float *taper_dev, int32_t N, float *cbar_dev, int32_t L, void *cuda_stream);
 
 /* ---- scalar variant: one polarisation ------------------------------------------
  * The method as the paper derives it before the 2x2 substitution (Eq. 1-25);
@@ -177,13 +200,13 @@ int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *cu
  * = the XX plane of the 4-polarisation calls with Jones matrices g I_2.  Same plan object, same conventions.
  *   vis / vis_out [B][T][C] complex64, gains [slots][stations][N][N] complex64, grid [L][L] complex64,
  *   subgrids [P][N][N] complex64 (idg_grid_scalar / idg_degrid_scalar use the plan's scratch). */
-int idg_grid_scalar(const idg_plan *plan, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+int idg_grid_scalar(const idg_plan *plan, const float *uvw_dev, const void *vis_dev, const void *gains_dev, int32_t n_slots,
                     const float *taper_dev, void *grid_dev, void *cuda_stream);
-int idg_degrid_scalar(const idg_plan *plan, const float *uvw_dev, const void *grid_dev, const void *gains_dev,
+int idg_degrid_scalar(const idg_plan *plan, const float *uvw_dev, const void *grid_dev, const void *gains_dev, int32_t n_slots,
                       const float *taper_dev, void *vis_out_dev, void *cuda_stream);
-int idg_gridder_scalar(const idg_plan *plan, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+int idg_gridder_scalar(const idg_plan *plan, const float *uvw_dev, const void *vis_dev, const void *gains_dev, int32_t n_slots,
                        const float *taper_dev, void *subgrids_dev, void *cuda_stream);
-int idg_degridder_scalar(const idg_plan *plan, const float *uvw_dev, const void *subgrids_dev, const void *gains_dev,
+int idg_degridder_scalar(const idg_plan *plan, const float *uvw_dev, const void *subgrids_dev, const void *gains_dev, int32_t n_slots,
                          const float *taper_dev, void *vis_out_dev, void *cuda_stream);
 
 #ifdef __cplusplus

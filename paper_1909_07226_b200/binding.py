@@ -23,10 +23,11 @@ assert META_DTYPE.itemsize == 48
 
 EXPORTS = (
     "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_plan_create", "idg_plan_from_metadata",
-    "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_destroy", "idg_grid",
+    "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_aterm_slots", "idg_plan_w_offset",
+    "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
     "idg_adder", "idg_splitter", "idg_splitter_ifft", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
-    "idg_image_divide", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
+    "idg_image_divide", "idg_image_taper", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
 
 
 class IdgError(RuntimeError):
@@ -129,17 +130,16 @@ class Plan:
         return out
 
     def slots_needed(self) -> int:
-        """Number of A-term slots the plan indexes (max aterm_slot + 1); cached."""
-        if getattr(self, "_slots", None) is None:
-            meta = self.metadata()
-            if len(meta) == 0:
-                self._slots = 0
-            elif int(self.params.flags) & 2:      # IDG_PLAN_SPAN_ATERMS: the last timestep of a block decides
-                last = (meta["time_begin"] + meta["n_time"] - 1) // int(self.params.aterm_interval)
-                self._slots = int(last.max()) + 1
-            else:
-                self._slots = int(meta["aterm_slot"].max()) + 1
-        return self._slots
+        """Number of A-term slots the plan indexes (idg_plan_aterm_slots)."""
+        n = ctypes.c_int32()
+        _check(lib().idg_plan_aterm_slots(self.handle, ctypes.byref(n)), "idg_plan_aterm_slots")
+        return int(n.value)
+
+    def w_offset(self, w_index: int) -> float:
+        """w0 of a w layer (idg_plan_w_offset; Alg. 1, R4)."""
+        w0 = ctypes.c_double()
+        _check(lib().idg_plan_w_offset(self.handle, ctypes.c_int32(int(w_index)), ctypes.byref(w0)), "idg_plan_w_offset")
+        return float(w0.value)
 
     def subgrids(self) -> torch.Tensor:
         """The plan-owned [P][4][N][N] complex64 scratch as a tensor view (not owned by torch)."""
@@ -217,9 +217,6 @@ def _shape_check(plan: Plan, uvw=None, vis=None, aterms=None, taper=None, grid=N
         s = tuple(aterms.shape)
         if len(s) != 5 or s[1:] != (plan.n_stations, N, N, 4):
             raise IdgError("aterms shape %s != [slots][%d][%d][%d][4]" % (s, plan.n_stations, N, N))
-        need = plan.slots_needed()
-        if need > s[0]:
-            raise IdgError("aterms has %d slots, the plan needs %d" % (s[0], need))
     if taper is not None and tuple(taper.shape) != (N, N):
         raise IdgError("taper shape %s != (%d, %d)" % (tuple(taper.shape), N, N))
     if grid is not None and tuple(grid.shape) != (4, L, L):
@@ -235,7 +232,7 @@ def idg_grid(plan: Plan, uvw, vis, aterms, taper, grid, stream=None) -> None:
     """Alg. 1: gridder -> subgrid FFT -> adder; accumulates into ``grid``."""
     _shape_check(plan, uvw=uvw, vis=vis, aterms=aterms, taper=taper, grid=grid)
     _check(lib().idg_grid(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"),
-                          _dev(aterms, _C64, "aterms"), _dev(taper, _F32, "taper"),
+                          _dev(aterms, _C64, "aterms"), ctypes.c_int32(int(aterms.shape[0])), _dev(taper, _F32, "taper"),
                           _dev(grid, _C64, "grid"), _stream(stream)), "idg_grid")
 
 
@@ -243,14 +240,14 @@ def idg_degrid(plan: Plan, uvw, grid, aterms, taper, vis_out, stream=None) -> No
     """Alg. 2: splitter -> subgrid IFFT -> degridder; writes ``vis_out``."""
     _shape_check(plan, uvw=uvw, vis=vis_out, aterms=aterms, taper=taper, grid=grid)
     _check(lib().idg_degrid(plan.handle, _dev(uvw, _F32, "uvw"), _dev(grid, _C64, "grid"),
-                            _dev(aterms, _C64, "aterms"), _dev(taper, _F32, "taper"),
+                            _dev(aterms, _C64, "aterms"), ctypes.c_int32(int(aterms.shape[0])), _dev(taper, _F32, "taper"),
                             _dev(vis_out, _C64, "vis_out"), _stream(stream)), "idg_degrid")
 
 
 def idg_gridder(plan: Plan, uvw, vis, aterms, taper, subgrids, stream=None) -> None:
     _shape_check(plan, uvw=uvw, vis=vis, aterms=aterms, taper=taper, subgrids=subgrids)
     _check(lib().idg_gridder(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"),
-                             _dev(aterms, _C64, "aterms"), _dev(taper, _F32, "taper"),
+                             _dev(aterms, _C64, "aterms"), ctypes.c_int32(int(aterms.shape[0])), _dev(taper, _F32, "taper"),
                              _dev(subgrids, _C64, "subgrids"), _stream(stream)), "idg_gridder")
 
 
@@ -282,7 +279,7 @@ def idg_splitter_ifft(plan: Plan, grid, subgrids, stream=None) -> None:
 def idg_degridder(plan: Plan, uvw, subgrids, aterms, taper, vis_out, stream=None) -> None:
     _shape_check(plan, uvw=uvw, vis=vis_out, aterms=aterms, taper=taper, subgrids=subgrids)
     _check(lib().idg_degridder(plan.handle, _dev(uvw, _F32, "uvw"), _dev(subgrids, _C64, "subgrids"),
-                               _dev(aterms, _C64, "aterms"), _dev(taper, _F32, "taper"),
+                               _dev(aterms, _C64, "aterms"), ctypes.c_int32(int(aterms.shape[0])), _dev(taper, _F32, "taper"),
                                _dev(vis_out, _C64, "vis_out"), _stream(stream)), "idg_degridder")
 
 
@@ -342,13 +339,24 @@ def idg_image_divide(image, cbar, stream=None) -> None:
                                   _stream(stream)), "idg_image_divide")
 
 
+def idg_image_taper(taper, L: int, stream=None) -> torch.Tensor:
+    """c-bar [L][L] float32 from the [N][N] subgrid taper (idg_image_taper; section 4.2)."""
+    N = int(taper.shape[0])
+    if tuple(taper.shape) != (N, N):
+        raise IdgError("taper must be [N][N]")
+    out = torch.empty((int(L), int(L)), dtype=_F32, device=taper.device)
+    _check(lib().idg_image_taper(_dev(taper, _F32, "taper"), ctypes.c_int32(N), _dev(out, _F32, "cbar"),
+                                 ctypes.c_int32(int(L)), _stream(stream)), "idg_image_taper")
+    return out
+
+
 def _scalar_check(plan: Plan, uvw, vis, gains, taper, grid=None, subgrids=None):
     N, L = int(plan.params.subgrid_size), int(plan.params.grid_size)
     if tuple(uvw.shape) != (plan.B, plan.T, 3) or tuple(vis.shape) != (plan.B, plan.T, plan.C):
         raise IdgError("scalar variant: uvw must be [B][T][3] and vis [B][T][C]")
     g = tuple(gains.shape)
-    if len(g) != 4 or g[1:] != (plan.n_stations, N, N) or g[0] < plan.slots_needed():
-        raise IdgError("scalar variant: gains must be [slots >= %d][%d][%d][%d]" % (plan.slots_needed(), plan.n_stations, N, N))
+    if len(g) != 4 or g[1:] != (plan.n_stations, N, N):
+        raise IdgError("scalar variant: gains must be [slots][%d][%d][%d]" % (plan.n_stations, N, N))
     if tuple(taper.shape) != (N, N):
         raise IdgError("taper shape")
     if grid is not None and tuple(grid.shape) != (L, L):
@@ -360,20 +368,20 @@ def _scalar_check(plan: Plan, uvw, vis, gains, taper, grid=None, subgrids=None):
 def idg_grid_scalar(plan: Plan, uvw, vis, gains, taper, grid, stream=None) -> None:
     """Scalar (one polarisation) Alg. 1; accumulates into grid [L][L] (NEXT-3)."""
     _scalar_check(plan, uvw, vis, gains, taper, grid=grid)
-    _check(lib().idg_grid_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"), _dev(gains, _C64, "gains"),
+    _check(lib().idg_grid_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"), _dev(gains, _C64, "gains"), ctypes.c_int32(int(gains.shape[0])),
                                  _dev(taper, _F32, "taper"), _dev(grid, _C64, "grid"), _stream(stream)), "idg_grid_scalar")
 
 
 def idg_degrid_scalar(plan: Plan, uvw, grid, gains, taper, vis_out, stream=None) -> None:
     _scalar_check(plan, uvw, vis_out, gains, taper, grid=grid)
-    _check(lib().idg_degrid_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(grid, _C64, "grid"), _dev(gains, _C64, "gains"),
+    _check(lib().idg_degrid_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(grid, _C64, "grid"), _dev(gains, _C64, "gains"), ctypes.c_int32(int(gains.shape[0])),
                                    _dev(taper, _F32, "taper"), _dev(vis_out, _C64, "vis_out"), _stream(stream)),
            "idg_degrid_scalar")
 
 
 def idg_gridder_scalar(plan: Plan, uvw, vis, gains, taper, subgrids, stream=None) -> None:
     _scalar_check(plan, uvw, vis, gains, taper, subgrids=subgrids)
-    _check(lib().idg_gridder_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"), _dev(gains, _C64, "gains"),
+    _check(lib().idg_gridder_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(vis, _C64, "vis"), _dev(gains, _C64, "gains"), ctypes.c_int32(int(gains.shape[0])),
                                     _dev(taper, _F32, "taper"), _dev(subgrids, _C64, "subgrids"), _stream(stream)),
            "idg_gridder_scalar")
 
@@ -381,5 +389,5 @@ def idg_gridder_scalar(plan: Plan, uvw, vis, gains, taper, subgrids, stream=None
 def idg_degridder_scalar(plan: Plan, uvw, subgrids, gains, taper, vis_out, stream=None) -> None:
     _scalar_check(plan, uvw, vis_out, gains, taper, subgrids=subgrids)
     _check(lib().idg_degridder_scalar(plan.handle, _dev(uvw, _F32, "uvw"), _dev(subgrids, _C64, "subgrids"),
-                                      _dev(gains, _C64, "gains"), _dev(taper, _F32, "taper"),
+                                      _dev(gains, _C64, "gains"), ctypes.c_int32(int(gains.shape[0])), _dev(taper, _F32, "taper"),
                                       _dev(vis_out, _C64, "vis_out"), _stream(stream)), "idg_degridder_scalar")

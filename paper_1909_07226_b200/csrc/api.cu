@@ -2,6 +2,7 @@
 #include <algorithm>
 #include <atomic>
 #include <cmath>
+#include <climits>
 #include <cstring>
 #include <new>
 
@@ -40,6 +41,7 @@ static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
       for (int tx = m.x0 / TX; tx <= (m.x0 + N - 1) / TX; ++tx) ++offs[(size_t)ty * ntx + tx + 1];
   for (size_t i = 1; i < offs.size(); ++i) offs[i] += offs[i - 1];
   const int64_t total = offs.back();
+  if (total > (int64_t)INT32_MAX) return IDG_ERR_INVALID_ARG;   // AdderItem ranges are int32
   std::vector<int32_t> list((size_t)total);
   std::vector<int64_t> cur(offs.begin(), offs.end() - 1);
   for (int64_t p = 0; p < pl->P; ++p) {
@@ -91,10 +93,17 @@ static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
 static int finish_plan(idg_plan *pl, const double *freqs_host, cudaStream_t stream) {
   const int N = pl->prm.subgrid_size;
   pl->P = (int64_t)pl->meta_host.size();
-  pl->max_n_time = 0; pl->max_n_chan = 0;
+  pl->max_n_time = 0; pl->max_n_chan = 0; pl->n_slots_needed = 0;
+  pl->sorted_by_baseline = true;
+  const bool span = (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
+  int32_t prev_b = 0;
   for (const auto &m : pl->meta_host) {
     pl->max_n_time = std::max(pl->max_n_time, m.n_time);
     pl->max_n_chan = std::max(pl->max_n_chan, m.n_chan);
+    const int32_t last = span ? (m.time_begin + m.n_time - 1) / pl->prm.aterm_interval : m.aterm_slot;
+    pl->n_slots_needed = std::max(pl->n_slots_needed, last + 1);
+    if (m.baseline < prev_b) pl->sorted_by_baseline = false;
+    prev_b = m.baseline;
   }
   // fraction of idle channel slots in the degridder if every thread owns cpt = 1, 2, 4, 8 channels of a timestep
   for (int k = 0; k < 4; ++k) {
@@ -175,6 +184,7 @@ void idg_plan_destroy(idg_plan *pl) {
 int idg_plan_create(idg_plan **out, const idg_plan_params *prm, const float *uvw_dev,
                     const double *freqs_host, const int32_t *baselines_host, int32_t B, int32_t T,
                     int32_t C, int32_t n_stations, void *cuda_stream) {
+  IDG_API_TRY
   if (out) *out = nullptr;
   if (!out || !uvw_dev || !freqs_host || !baselines_host || B < 1 || T < 1 || C < 1 || n_stations < 1)
     return IDG_ERR_INVALID_ARG;
@@ -187,18 +197,25 @@ int idg_plan_create(idg_plan **out, const idg_plan_params *prm, const float *uvw
   idg_plan *pl = new (std::nothrow) idg_plan();
   if (!pl) return IDG_ERR_OUT_OF_MEMORY;
   pl->prm = *prm; pl->B = B; pl->T = T; pl->C = C; pl->n_stations = n_stations;
+  pl->planner_made = true;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
-  rc = run_planner(*prm, uvw_dev, freqs_host, baselines_host, B, T, C, pl->meta_host, &pl->meta_dev,
-                   &pl->n_planned, &pl->n_skipped, stream);
-  if (rc == IDG_OK) rc = finish_plan(pl, freqs_host, stream);
+  try {
+    rc = run_planner(*prm, uvw_dev, freqs_host, baselines_host, B, T, C, pl->meta_host, &pl->meta_dev,
+                     &pl->n_planned, &pl->n_skipped, stream);
+  } catch (const std::bad_alloc &) { rc = IDG_ERR_OUT_OF_MEMORY; }
+  if (rc == IDG_OK) {
+    try { rc = finish_plan(pl, freqs_host, stream); } catch (const std::bad_alloc &) { rc = IDG_ERR_OUT_OF_MEMORY; }
+  }
   if (rc != IDG_OK) { idg_plan_destroy(pl); return rc; }
   *out = pl;
   return IDG_OK;
+  IDG_API_CATCH
 }
 
 int idg_plan_from_metadata(idg_plan **out, const idg_plan_params *prm,
                            const idg_subgrid_meta *meta_host, int64_t P, const double *freqs_host,
                            int32_t B, int32_t T, int32_t C, int32_t n_stations, void *cuda_stream) {
+  IDG_API_TRY
   if (out) *out = nullptr;
   if (!out || (!meta_host && P > 0) || P < 0 || !freqs_host || B < 1 || T < 1 || C < 1 || n_stations < 1)
     return IDG_ERR_INVALID_ARG;
@@ -208,18 +225,21 @@ int idg_plan_from_metadata(idg_plan **out, const idg_plan_params *prm,
   int64_t planned = 0;
   for (int64_t p = 0; p < P; ++p) {
     const idg_subgrid_meta &m = meta_host[p];
-    const bool ok = m.baseline >= 0 && m.baseline < B && m.station1 >= 0 && m.station1 < n_stations &&
-                    m.station2 >= 0 && m.station2 < n_stations && m.time_begin >= 0 && m.n_time >= 1 &&
-                    m.time_begin + m.n_time <= T && m.chan_begin >= 0 && m.n_chan >= 1 &&
-                    m.n_chan <= 256 && m.chan_begin + m.n_chan <= C && m.aterm_slot >= 0 &&
-                    m.x0 >= 0 && m.y0 >= 0 && m.x0 + N <= L && m.y0 + N <= L;
+    // ranges in int64: time_begin + n_time may not wrap past the <= T check
+    bool ok = m.baseline >= 0 && m.baseline < B && m.station1 >= 0 && m.station1 < n_stations &&
+              m.station2 >= 0 && m.station2 < n_stations && m.time_begin >= 0 && m.n_time >= 1 &&
+              (int64_t)m.time_begin + m.n_time <= T && m.chan_begin >= 0 && m.n_chan >= 1 &&
+              m.n_chan <= 256 && (int64_t)m.chan_begin + m.n_chan <= C && m.aterm_slot >= 0 &&
+              m.x0 >= 0 && m.y0 >= 0 && (int64_t)m.x0 + N <= L && (int64_t)m.y0 + N <= L;
+    // with IDG_PLAN_SPAN_ATERMS the kernels walk the slots from aterm_slot on: it must be the first timestep's
+    if (ok && (prm->flags & IDG_PLAN_SPAN_ATERMS)) ok = m.aterm_slot == m.time_begin / prm->aterm_interval;
     if (!ok) return IDG_ERR_PLAN_MISMATCH;
     planned += (int64_t)m.n_time * m.n_chan;
   }
   idg_plan *pl = new (std::nothrow) idg_plan();
   if (!pl) return IDG_ERR_OUT_OF_MEMORY;
   pl->prm = *prm; pl->B = B; pl->T = T; pl->C = C; pl->n_stations = n_stations;
-  pl->meta_host.assign(meta_host, meta_host + P);
+  try { pl->meta_host.assign(meta_host, meta_host + P); } catch (const std::bad_alloc &) { delete pl; return IDG_ERR_OUT_OF_MEMORY; }
   pl->n_planned = planned;
   pl->n_skipped = (int64_t)B * T * C - planned;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
@@ -232,10 +252,13 @@ int idg_plan_from_metadata(idg_plan **out, const idg_plan_params *prm,
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) { set_last_cuda_error(e); rc = IDG_ERR_CUDA; }
   }
-  if (rc == IDG_OK) rc = finish_plan(pl, freqs_host, stream);
+  if (rc == IDG_OK) {
+    try { rc = finish_plan(pl, freqs_host, stream); } catch (const std::bad_alloc &) { rc = IDG_ERR_OUT_OF_MEMORY; }
+  }
   if (rc != IDG_OK) { idg_plan_destroy(pl); return rc; }
   *out = pl;
   return IDG_OK;
+  IDG_API_CATCH
 }
 
 int idg_plan_size(const idg_plan *pl, int64_t *n_subgrids, int64_t *n_planned_vis,
@@ -256,6 +279,18 @@ int idg_plan_metadata(const idg_plan *pl, idg_subgrid_meta *out_host, int64_t ca
 int idg_plan_subgrids(const idg_plan *pl, void **subgrids_dev) {
   if (!pl || !subgrids_dev) return IDG_ERR_INVALID_ARG;
   *subgrids_dev = pl->subgrids_dev;
+  return IDG_OK;
+}
+
+int idg_plan_aterm_slots(const idg_plan *pl, int32_t *n_slots) {
+  if (!pl || !n_slots) return IDG_ERR_INVALID_ARG;
+  *n_slots = pl->n_slots_needed;
+  return IDG_OK;
+}
+
+int idg_plan_w_offset(const idg_plan *pl, int32_t w_index, double *w0) {
+  if (!pl || !w0) return IDG_ERR_INVALID_ARG;
+  *w0 = pl->prm.w_step > 0.0 ? ((double)w_index + 0.5) * pl->prm.w_step : 0.0;   // R4
   return IDG_OK;
 }
 

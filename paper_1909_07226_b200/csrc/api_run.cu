@@ -38,16 +38,6 @@ int ensure_staging(idg_plan *pl, int32_t n_slots) {
   return IDG_OK;
 }
 
-int needed_slots(const idg_plan *pl) {
-  int s = 0;
-  const bool span = (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
-  for (const auto &m : pl->meta_host) {
-    const int last = span ? (m.time_begin + m.n_time - 1) / pl->prm.aterm_interval : m.aterm_slot;
-    s = last + 1 > s ? last + 1 : s;
-  }
-  return s;
-}
-
 // The host-buffer calls overlap the PCIe copies with the kernels: the baselines are cut into kHostChunks
 // contiguous ranges (the metadata is sorted by baseline, so a range of baselines is a range of subgrids and a
 // contiguous slice of vis); uploads run on the plan's copy stream, kernels on the caller's stream, events
@@ -64,7 +54,9 @@ int ensure_host_pipeline(idg_plan *pl) {
 
 std::vector<HostChunk> host_chunks(const idg_plan *pl) {
   std::vector<HostChunk> out;
-  const int n = std::min<int>(idg_plan::kHostChunks, pl->B);
+  // metadata given through idg_plan_from_metadata may come in any order: a baseline range is then no subgrid range
+  // and the calls run as one chunk (everything uploaded, then computed, then copied back)
+  const int n = pl->sorted_by_baseline ? std::min<int>(idg_plan::kHostChunks, pl->B) : 1;
   int64_t p = 0;
   for (int k = 0; k < n; ++k) {
     HostChunk c;
@@ -84,15 +76,17 @@ std::vector<HostChunk> host_chunks(const idg_plan *pl) {
 extern "C" {
 
 int idg_gridder(const idg_plan *pl, const float *uvw_dev, const void *vis_dev,
-                const void *aterms_dev, const float *taper_dev, void *subgrids_dev, void *stream) {
+                const void *aterms_dev, int32_t n_slots, const float *taper_dev, void *subgrids_dev, void *stream) {
   if (!pl || !uvw_dev || !vis_dev || !aterms_dev || !taper_dev || (!subgrids_dev && pl->P > 0))
     return IDG_ERR_INVALID_ARG;
+  if (!aligned16(vis_dev) || !aligned16(aterms_dev) || !aligned16(subgrids_dev)) return IDG_ERR_INVALID_ARG;
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   return launch_gridder(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)aterms_dev, taper_dev,
                         (float2 *)subgrids_dev, S(stream));
 }
 
 int idg_subgrid_fft(const idg_plan *pl, void *subgrids_dev, int32_t direction, void *stream) {
-  if (!pl || (!subgrids_dev && pl->P > 0) || (direction != -1 && direction != 1))
+  if (!pl || (!subgrids_dev && pl->P > 0) || (direction != -1 && direction != 1) || !aligned16(subgrids_dev))
     return IDG_ERR_INVALID_ARG;
   return launch_subgrid_fft(pl, (float2 *)subgrids_dev, direction, S(stream));
 }
@@ -113,16 +107,20 @@ int idg_splitter_ifft(const idg_plan *pl, const void *grid_dev, void *subgrids_d
 }
 
 int idg_degridder(const idg_plan *pl, const float *uvw_dev, const void *subgrids_dev,
-                  const void *aterms_dev, const float *taper_dev, void *vis_out_dev, void *stream) {
+                  const void *aterms_dev, int32_t n_slots, const float *taper_dev, void *vis_out_dev, void *stream) {
   if (!pl || !uvw_dev || (!subgrids_dev && pl->P > 0) || !aterms_dev || !taper_dev || !vis_out_dev)
     return IDG_ERR_INVALID_ARG;
+  if (!aligned16(vis_out_dev) || !aligned16(aterms_dev) || !aligned16(subgrids_dev)) return IDG_ERR_INVALID_ARG;
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   return launch_degridder(pl, uvw_dev, (const float2 *)subgrids_dev, (const float2 *)aterms_dev,
                           taper_dev, (float2 *)vis_out_dev, S(stream));
 }
 
 int idg_grid(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *aterms_dev,
-             const float *taper_dev, void *grid_dev, void *stream) {
+             int32_t n_slots, const float *taper_dev, void *grid_dev, void *stream) {
   if (!pl || !uvw_dev || !vis_dev || !aterms_dev || !taper_dev || !grid_dev) return IDG_ERR_INVALID_ARG;
+  if (!aligned16(vis_dev) || !aligned16(aterms_dev)) return IDG_ERR_INVALID_ARG;
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   int rc = launch_gridder(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)aterms_dev, taper_dev,
                           pl->subgrids_dev, S(stream));
   if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, -1, S(stream));
@@ -131,9 +129,13 @@ int idg_grid(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, cons
 }
 
 int idg_degrid(const idg_plan *pl, const float *uvw_dev, const void *grid_dev,
-               const void *aterms_dev, const float *taper_dev, void *vis_out_dev, void *stream) {
+               const void *aterms_dev, int32_t n_slots, const float *taper_dev, void *vis_out_dev, void *stream) {
   if (!pl || !uvw_dev || !grid_dev || !aterms_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
-  if (pl->n_skipped > 0)  // skipped samples read as 0; planned ones are overwritten below
+  if (!aligned16(vis_out_dev) || !aligned16(aterms_dev)) return IDG_ERR_INVALID_ARG;
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
+  // skipped samples read as 0; planned ones are overwritten below.  Only the planner guarantees that every sample
+  // is covered exactly once or counted skipped; caller-made metadata may overlap, so its output is always zeroed.
+  if (pl->n_skipped > 0 || !pl->planner_made)
     IDG_CUDA_TRY(cudaMemsetAsync(vis_out_dev, 0, sizeof(float2) * 4 * (size_t)pl->B * pl->T * pl->C, S(stream)));
   int rc = launch_splitter_ifft(pl, (const float2 *)grid_dev, pl->subgrids_dev, S(stream));
   if (rc == IDG_OK)
@@ -144,26 +146,29 @@ int idg_degrid(const idg_plan *pl, const float *uvw_dev, const void *grid_dev,
 
 // ---- scalar variant (NEXT-3): one polarisation; subgrids [P][N][N] live in the first quarter of the plan's
 // scratch; the plane-wise FFT kernel sees them as ceil(P / 4) four-plane subgrids ------------------------------
-int idg_gridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+int idg_gridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev, int32_t n_slots,
                        const float *taper_dev, void *subgrids_dev, void *stream) {
   if (!pl || !uvw_dev || !vis_dev || !gains_dev || !taper_dev || (!subgrids_dev && pl->P > 0)) return IDG_ERR_INVALID_ARG;
   if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   return launch_gridder_scalar(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)gains_dev, taper_dev,
                                (float2 *)subgrids_dev, S(stream));
 }
 
-int idg_degridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *subgrids_dev, const void *gains_dev,
+int idg_degridder_scalar(const idg_plan *pl, const float *uvw_dev, const void *subgrids_dev, const void *gains_dev, int32_t n_slots,
                          const float *taper_dev, void *vis_out_dev, void *stream) {
   if (!pl || !uvw_dev || (!subgrids_dev && pl->P > 0) || !gains_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
   if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   return launch_degridder_scalar(pl, uvw_dev, (const float2 *)subgrids_dev, (const float2 *)gains_dev, taper_dev,
                                  (float2 *)vis_out_dev, S(stream));
 }
 
-int idg_grid_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev,
+int idg_grid_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_dev, const void *gains_dev, int32_t n_slots,
                     const float *taper_dev, void *grid_dev, void *stream) {
   if (!pl || !uvw_dev || !vis_dev || !gains_dev || !taper_dev || !grid_dev) return IDG_ERR_INVALID_ARG;
   if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   int rc = launch_gridder_scalar(pl, uvw_dev, (const float2 *)vis_dev, (const float2 *)gains_dev, taper_dev,
                                  pl->subgrids_dev, S(stream));
   if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, -1, S(stream), 0, (pl->P + 3) / 4);
@@ -171,11 +176,12 @@ int idg_grid_scalar(const idg_plan *pl, const float *uvw_dev, const void *vis_de
   return rc;
 }
 
-int idg_degrid_scalar(const idg_plan *pl, const float *uvw_dev, const void *grid_dev, const void *gains_dev,
+int idg_degrid_scalar(const idg_plan *pl, const float *uvw_dev, const void *grid_dev, const void *gains_dev, int32_t n_slots,
                       const float *taper_dev, void *vis_out_dev, void *stream) {
   if (!pl || !uvw_dev || !grid_dev || !gains_dev || !taper_dev || !vis_out_dev) return IDG_ERR_INVALID_ARG;
   if (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) return IDG_ERR_PLAN_MISMATCH;   // scalar kernels are per-block c_p only
-  if (pl->n_skipped > 0)
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
+  if (pl->n_skipped > 0 || !pl->planner_made)
     IDG_CUDA_TRY(cudaMemsetAsync(vis_out_dev, 0, sizeof(float2) * (size_t)pl->B * pl->T * pl->C, S(stream)));
   int rc = launch_splitter(pl, (const float2 *)grid_dev, pl->subgrids_dev, S(stream), 0, -1, 1);
   if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, +1, S(stream), 0, (pl->P + 3) / 4);
@@ -185,11 +191,11 @@ int idg_degrid_scalar(const idg_plan *pl, const float *uvw_dev, const void *grid
   return rc;
 }
 
-int idg_grid_host(idg_plan *pl, const float *uvw_host, const void *vis_host,
+static int grid_host_impl(idg_plan *pl, const float *uvw_host, const void *vis_host,
                   const void *aterms_host, int32_t n_slots, const float *taper_host,
                   void *grid_host, void *stream) {
   if (!pl || !uvw_host || !vis_host || !aterms_host || !taper_host || !grid_host) return IDG_ERR_INVALID_ARG;
-  if (n_slots < needed_slots(pl)) return IDG_ERR_PLAN_MISMATCH;
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   int rc = ensure_staging(pl, n_slots);
   if (rc == IDG_OK) rc = ensure_host_pipeline(pl);
   if (rc != IDG_OK) return rc;
@@ -231,11 +237,11 @@ int idg_grid_host(idg_plan *pl, const float *uvw_host, const void *vis_host,
   return IDG_OK;
 }
 
-int idg_degrid_host(idg_plan *pl, const float *uvw_host, const void *grid_host,
+static int degrid_host_impl(idg_plan *pl, const float *uvw_host, const void *grid_host,
                     const void *aterms_host, int32_t n_slots, const float *taper_host,
                     void *vis_out_host, void *stream) {
   if (!pl || !uvw_host || !vis_out_host || !aterms_host || !taper_host || !grid_host) return IDG_ERR_INVALID_ARG;
-  if (n_slots < needed_slots(pl)) return IDG_ERR_PLAN_MISMATCH;
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
   int rc = ensure_staging(pl, n_slots);
   if (rc == IDG_OK) rc = ensure_host_pipeline(pl);
   if (rc != IDG_OK) return rc;
@@ -249,7 +255,7 @@ int idg_degrid_host(idg_plan *pl, const float *uvw_host, const void *grid_host,
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_aterms_dev, aterms_host, sizeof(float2) * 4 * N * N * (size_t)pl->n_stations * n_slots, cudaMemcpyHostToDevice, s));
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_taper_dev, taper_host, sizeof(float) * N * N, cudaMemcpyHostToDevice, s));
   IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_grid_dev, grid_host, sizeof(float2) * 4 * L * L, cudaMemcpyHostToDevice, s));
-  if (pl->n_skipped > 0)   // skipped samples read as 0; planned ones are overwritten below
+  if (pl->n_skipped > 0 || !pl->planner_made)   // skipped samples read as 0; planned ones are overwritten below
     IDG_CUDA_TRY(cudaMemsetAsync(pl->h_vis_dev, 0, sizeof(float2) * 4 * nvis, s));
   for (size_t k = 0; k < chunks.size(); ++k) {
     const HostChunk &ch = chunks[k];
@@ -266,6 +272,34 @@ int idg_degrid_host(idg_plan *pl, const float *uvw_host, const void *grid_host,
   IDG_CUDA_TRY(cudaStreamSynchronize(s));
   IDG_CUDA_TRY(cudaStreamSynchronize(c));
   return IDG_OK;
+}
+
+// On failure the asynchronous copies already queued still reference the caller's host buffers: both streams are
+// drained before the error is returned, so the caller may free them.
+static int host_call_epilogue(idg_plan *pl, void *stream, int rc) {
+  if (rc != IDG_OK && pl) {
+    cudaStreamSynchronize(S(stream));
+    if (pl->h_copy_stream) cudaStreamSynchronize(pl->h_copy_stream);
+  }
+  return rc;
+}
+
+int idg_grid_host(idg_plan *pl, const float *uvw_host, const void *vis_host, const void *aterms_host, int32_t n_slots,
+                  const float *taper_host, void *grid_host, void *stream) {
+  int rc;
+  try {
+    rc = grid_host_impl(pl, uvw_host, vis_host, aterms_host, n_slots, taper_host, grid_host, stream);
+  } catch (const std::bad_alloc &) { rc = IDG_ERR_OUT_OF_MEMORY; } catch (...) { rc = IDG_ERR_INVALID_ARG; }
+  return host_call_epilogue(pl, stream, rc);
+}
+
+int idg_degrid_host(idg_plan *pl, const float *uvw_host, const void *grid_host, const void *aterms_host,
+                    int32_t n_slots, const float *taper_host, void *vis_out_host, void *stream) {
+  int rc;
+  try {
+    rc = degrid_host_impl(pl, uvw_host, grid_host, aterms_host, n_slots, taper_host, vis_out_host, stream);
+  } catch (const std::bad_alloc &) { rc = IDG_ERR_OUT_OF_MEMORY; } catch (...) { rc = IDG_ERR_INVALID_ARG; }
+  return host_call_epilogue(pl, stream, rc);
 }
 
 }  // extern "C"

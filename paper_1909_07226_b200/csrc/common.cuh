@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <new>
 #include <vector>
 
 #include "../../include/idg_b200.h"
@@ -28,6 +29,9 @@ struct idg_plan {
   int32_t B = 0, T = 0, C = 0, n_stations = 0;
   int64_t P = 0, n_planned = 0, n_skipped = 0;
   int32_t max_n_time = 0, max_n_chan = 0;
+  int32_t n_slots_needed = 0;         // A-term slots the metadata indexes (last slot + 1)
+  bool planner_made = false;          // metadata from run_planner: sorted by baseline, every sample covered once or skipped
+  bool sorted_by_baseline = false;    // baselines non-decreasing in metadata order (the *_host calls chunk by baseline)
   float dg_waste[4] = {0.f, 0.f, 0.f, 0.f};   // degridder: idle channel slots if threads own 1, 2, 4, 8 channels
   float uniform_dkd = 0.f;            // 2 pi df / c0 when the channels are equally spaced, else 0 (scalar.cu)
   std::vector<idg_subgrid_meta> meta_host;
@@ -72,6 +76,15 @@ void count_launch();
     idg::count_launch();               \
     IDG_CUDA_TRY(cudaGetLastError()); \
   } while (0)
+
+// extern "C" bodies: nothing may throw across the C boundary (std::vector growth inside the library)
+#define IDG_API_TRY try {
+#define IDG_API_CATCH                                         \
+  }                                                           \
+  catch (const std::bad_alloc &) { return IDG_ERR_OUT_OF_MEMORY; } \
+  catch (...) { return IDG_ERR_INVALID_ARG; }
+
+inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 // planner (plan.cu)
 int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *freqs_host,

@@ -28,7 +28,7 @@ __device__ __forceinline__ float2 w_phasor(int x, int y, int L, double image_siz
 
 template <bool ACCUMULATE>
 __global__ void __launch_bounds__(256)
-image_w_kernel(float2 *__restrict__ dst, const float2 *__restrict__ src, int L, double image_size,
+image_w_kernel(float2 *dst, const float2 *src, int L, double image_size,   // out may alias in: no __restrict__
                double w0, double sign) {
   const int x = blockIdx.x * 64 + (threadIdx.x & 63);
   const int y = blockIdx.y * 4 + (threadIdx.x >> 6);
@@ -56,6 +56,56 @@ image_divide_kernel(float2 *__restrict__ image, const float *__restrict__ cbar, 
     v.x *= inv; v.y *= inv;
     image[i] = v;
   }
+}
+
+// ---- c-bar: the subgrid taper on the image raster (idg_image_taper) ---------------------------------------------
+// Section 4.2: the window the method effectively applies is the periodic sinc (Dirichlet kernel)
+// interpolation of the discrete taper; at zero shift that interpolant, evaluated at the L image pixels, is c-bar:
+//   D(x, i)    = (1/N) sum_{a=-N/2}^{N/2-1} exp(2 pi i a ((x - L/2)/L - (i - N/2)/N))
+//   cbar[y][x] = Re sum_{j,i} D(y, j) taper[j][i] D(x, i)
+// Three small FP64 kernels: the table D [L][N], tmp = D taper [L][N], cbar = Re(tmp D^T) [L][L].
+__global__ void __launch_bounds__(128)
+taper_dirichlet_kernel(double2 *__restrict__ D, int N, int L) {
+  const int idx = blockIdx.x * 128 + threadIdx.x;
+  if (idx >= L * N) return;
+  const int x = idx / N, i = idx - x * N;
+  const double delta = (double)(x - L / 2) / (double)L - (double)(i - N / 2) / (double)N;
+  double re = 0.0, im = 0.0;
+  for (int a = -N / 2; a < N / 2; ++a) {
+    double s, c;
+    sincospi(2.0 * (double)a * delta, &s, &c);
+    re += c; im += s;
+  }
+  D[idx] = make_double2(re / (double)N, im / (double)N);
+}
+
+__global__ void __launch_bounds__(128)
+taper_rows_kernel(double2 *__restrict__ tmp, const double2 *__restrict__ D, const float *__restrict__ taper, int N,
+                  int L) {
+  const int idx = blockIdx.x * 128 + threadIdx.x;
+  if (idx >= L * N) return;
+  const int y = idx / N, i = idx - y * N;
+  double re = 0.0, im = 0.0;
+  for (int j = 0; j < N; ++j) {
+    const double2 d = D[y * N + j];
+    const double t = (double)taper[j * N + i];
+    re += d.x * t; im += d.y * t;
+  }
+  tmp[idx] = make_double2(re, im);
+}
+
+__global__ void __launch_bounds__(256)
+taper_image_kernel(float *__restrict__ cbar, const double2 *__restrict__ tmp, const double2 *__restrict__ D, int N,
+                   int L) {
+  const int x = blockIdx.x * 64 + (threadIdx.x & 63);
+  const int y = blockIdx.y * 4 + (threadIdx.x >> 6);
+  if (x >= L || y >= L) return;
+  double re = 0.0;
+  for (int i = 0; i < N; ++i) {
+    const double2 t = tmp[y * N + i], d = D[x * N + i];
+    re += t.x * d.x - t.y * d.y;
+  }
+  cbar[(size_t)y * L + x] = (float)re;
 }
 
 }  // namespace idg
@@ -89,6 +139,26 @@ int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *st
   const dim3 grid((L + 63) / 64, (L + 3) / 4);
   image_divide_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((float2 *)image_dev, cbar_dev, L);
   IDG_LAUNCH_CHECK();
+  return IDG_OK;
+}
+
+int idg_image_taper(const float *taper_dev, int32_t N, float *cbar_dev, int32_t L, void *stream) {
+  if (!taper_dev || !cbar_dev || !(N == 16 || N == 24 || N == 32 || N == 48) || L < N || (L & 1))
+    return IDG_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  double2 *D = nullptr, *tmp = nullptr;
+  IDG_CUDA_TRY(cudaMallocAsync(&D, sizeof(double2) * (size_t)L * N * 2, s));
+  tmp = D + (size_t)L * N;
+  const int nb = (L * N + 127) / 128;
+  taper_dirichlet_kernel<<<nb, 128, 0, s>>>(D, N, L);
+  count_launch();
+  taper_rows_kernel<<<nb, 128, 0, s>>>(tmp, D, taper_dev, N, L);
+  count_launch();
+  taper_image_kernel<<<dim3((L + 63) / 64, (L + 3) / 4), 256, 0, s>>>(cbar_dev, tmp, D, N, L);
+  count_launch();
+  const cudaError_t e = cudaGetLastError();
+  cudaFreeAsync(D, s);
+  IDG_CUDA_TRY(e);
   return IDG_OK;
 }
 

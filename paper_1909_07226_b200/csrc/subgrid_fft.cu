@@ -31,7 +31,9 @@ subgrid_fft_kernel(float2 *__restrict__ subgrids, const idg_subgrid_meta *__rest
 
   if (GATHER) {
     const int x0 = meta[blockIdx.x].x0, y0 = meta[blockIdx.x].y0;
-    if (((x0 | L) & 1) == 0) {     // window rows start on 16-byte boundaries: two pixels per load
+    // window rows start on 16-byte boundaries (x0 and L even, and the caller's grid itself 16-byte aligned -- the
+    // header asks only for 8): two pixels per load
+    if (((x0 | L) & 1) == 0 && (reinterpret_cast<uintptr_t>(grid) & 15u) == 0) {
 #pragma unroll 8
       for (int i = tid; i < 2 * N * N; i += 4 * N) {
         const int e = 2 * i;

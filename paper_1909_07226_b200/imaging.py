@@ -32,16 +32,8 @@ def _centred_fft2(img: torch.Tensor) -> torch.Tensor:
 
 
 def image_taper(taper: torch.Tensor, L: int) -> torch.Tensor:
-    """c-bar [L][L] float32: the [N][N] subgrid taper carried to the image raster by trigonometric
-    interpolation (section 4.2): zero-pad its centred DFT to L x L and transform back (library FFT)."""
-    N = int(taper.shape[0])
-    t = taper.to(torch.complex128)
-    coef = torch.fft.fftshift(torch.fft.fft2(torch.fft.ifftshift(t)), dim=(-2, -1)) / (N * N)
-    pad = torch.zeros((L, L), dtype=torch.complex128, device=taper.device)
-    o = L // 2 - N // 2
-    pad[o:o + N, o:o + N] = coef
-    cb = torch.fft.fftshift(torch.fft.ifft2(torch.fft.ifftshift(pad), norm="forward"), dim=(-2, -1))
-    return cb.real.to(torch.float32).contiguous()
+    """c-bar [L][L] float32 (idg_image_taper: the subgrid taper on the image raster)."""
+    return idg.idg_image_taper(taper, L)
 
 
 def layer_plans(params, uvw: torch.Tensor, freqs, baselines, n_stations: int) -> List[Tuple[int, float, "idg.Plan"]]:
@@ -53,8 +45,8 @@ def layer_plans(params, uvw: torch.Tensor, freqs, baselines, n_stations: int) ->
     out = []
     for wi in np.unique(meta["w_index"]):
         sel = np.ascontiguousarray(meta[meta["w_index"] == wi])
-        w0 = (int(wi) + 0.5) * float(params.w_step) if params.w_step > 0 else 0.0
-        out.append((int(wi), w0, idg.idg_plan_from_metadata(params, sel, freqs, B, T, n_stations)))
+        layer = idg.idg_plan_from_metadata(params, sel, freqs, B, T, n_stations)
+        out.append((int(wi), layer.w_offset(int(wi)), layer))
     return out
 
 

@@ -567,15 +567,6 @@ def test_scalar_variant_matches_xx_plane_of_the_oracle(name, kw, uneven):
     assert H.rel_l2(out.cpu().numpy(), ref_vis) < TOL
 
 
-def test_ska_full_size_sampled():
-    """BASELINE.json configs[2] and [3] at full size (8128 baselines, 133 M visibilities, 8192^2 grid, ~266 k
-    subgrids) in the launch configuration bench.py --workload ska times: plan bit-exact against the oracle planner,
-    24 sampled subgrids / blocks against the oracle in both directions, adder by conservation and sampled windows."""
-    w = synth.make_workload("ska", device="cuda")            # generated on the GPU (seconds), checked from a host copy
-    host = dataclasses.replace(w, uvw=w.uvw.cpu(), vis=w.vis.cpu(), aterms=w.aterms.cpu(), taper=w.taper.cpu())
-    assert _sampled_full_size_check(host, 24, 31) > 250000
-
-
 # ---------------------------------------------------------------------------------------------
 # NEXT-4: per-sample c_pk -- blocks that span A-term slots (IDG_PLAN_SPAN_ATERMS)
 # ---------------------------------------------------------------------------------------------
@@ -656,7 +647,7 @@ def test_error_paths_with_a_device(tiny_case):
     # too few A-term slots, wrong shapes, host tensors where device tensors are expected
     L = prm.grid_size
     g = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
-    with pytest.raises(idg.IdgError, match="slots"):
+    with pytest.raises(idg.IdgError, match="does not match"):     # refused by the C library (IDG_ERR_PLAN_MISMATCH)
         idg.idg_grid(c["plan"], c["wc"].uvw, c["wc"].vis, c["wc"].aterms[:1].contiguous(), c["wc"].taper, g)
     with pytest.raises(idg.IdgError, match="grid shape"):
         idg.idg_grid(c["plan"], c["wc"].uvw, c["wc"].vis, c["wc"].aterms, c["wc"].taper, g[:, :-1].contiguous())
