@@ -452,10 +452,11 @@ def run_b200(args):
     if clocks and clocks.get("sm_mhz"):
         roofline["frac_at_measured_clock"] = roofline["frac"] * (SM_MAX_HZ / 1e6) / clocks["sm_mhz"]
     try:     # the bare instruction mix of the inner loop, measured live (csrc/mixbench.cu): the practical ceiling
-        mix = idg.idg_bench_instruction_mix()
-        roofline["measured_mix_peak"] = {"tflops": mix, "frac_of_alu_peak": mix / ALU_PEAK_TFLOPS,
-                                         "gridder_frac_of_mix_peak": g["achieved"] / mix,
-                                         "what": "1 FFMA + sin/cos.approx + 8 FFMA2 per (visibility, pixel) on registers, no memory"}
+        mix = [idg.idg_bench_instruction_mix(4096, v) for v in (0, 1, 2)]
+        roofline["measured_mix_peak"] = {
+            "tflops": mix[0], "frac_of_alu_peak": mix[0] / ALU_PEAK_TFLOPS, "gridder_frac_of_mix_peak": g["achieved"] / mix[0],
+            "what": "1 FFMA + sin/cos.approx + 8 FFMA2 per (visibility, pixel), operands as in the gridder, no global memory",
+            "uniform_register_operands_tflops": mix[1], "scalar_ffma_tflops": mix[2]}
     except Exception as exc:      # reporting only
         roofline["measured_mix_peak"] = {"error": str(exc)}
     grid_bytes = 8.0 * 4 * L * L

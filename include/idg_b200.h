@@ -90,6 +90,15 @@ int idg_last_cuda_error(void);
  * the difference of two readings counts the launches in between.  Host-side bookkeeping only, never fails. */
 long long idg_kernel_launches(void);
 
+/* Measurement aid for the op-count roofline: runs the bare instruction mix of one
+ * (visibility, pixel) pair of Eq. 25 -- 1 FMA + sin/cos.approx + 16 FMA as packed pairs -- on
+ * registers and shared memory only, in the gridder's CTA shape, `iters` pairs per pixel, and returns the rate in
+ * TFLOP-equivalents/s (36 per pair, the unit of bench.py's roofline).  variant 0: operands as in the gridder
+ * (visibility pairs in vector registers, loaded from shared memory); 1: visibility pairs in uniform registers (an
+ * upper bound the real kernel cannot reach from CUDA C); 2: 16 scalar FMA instead of 8 packed ones.
+ * Synchronises cuda_stream; allocates and frees a small buffer. */
+int idg_bench_instruction_mix(int32_t iters, int32_t variant, double *tflop_equiv_per_s, void *cuda_stream);
+
 /* ---- planner (a0): section 3.2, Fig. 2; readings R10-R12 -----
  * Partitions every baseline's (time x channel) samples into blocks whose uv extent in grid
  * pixels plus kernel_size fits N, with one A-term slot and one w layer per block.  Runs on the

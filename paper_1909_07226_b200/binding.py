@@ -22,7 +22,7 @@ META_DTYPE = np.dtype([(n, "<i4") for n in (
 assert META_DTYPE.itemsize == 48
 
 EXPORTS = (
-    "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_plan_create", "idg_plan_from_metadata",
+    "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_bench_instruction_mix", "idg_plan_create", "idg_plan_from_metadata",
     "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_aterm_slots", "idg_plan_w_offset",
     "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
@@ -176,6 +176,15 @@ class _DevView:
 def idg_kernel_launches() -> int:
     """Kernels launched by the library in this process so far (host-side counter)."""
     return int(lib().idg_kernel_launches())
+
+
+def idg_bench_instruction_mix(iters: int = 4096, variant: int = 0, stream=None) -> float:
+    """TFLOP-equivalents/s of the bare gridder instruction mix on this device (csrc/mixbench.cu)."""
+    out = ctypes.c_double()
+    _check(lib().idg_bench_instruction_mix(ctypes.c_int32(int(iters)), ctypes.c_int32(int(variant)), ctypes.byref(out),
+                                           _stream(stream)),
+           "idg_bench_instruction_mix")
+    return float(out.value)
 
 
 def idg_plan_create(params, uvw: torch.Tensor, freqs, baselines, n_stations: int, stream=None) -> Plan:

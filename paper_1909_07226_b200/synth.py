@@ -266,16 +266,21 @@ def _stations(name: str, rng) -> np.ndarray:
     raise KeyError(name)
 
 
+def n_stations_of(name: str) -> int:
+    """Number of stations of a named workload (its baselines are all pairs, lexicographic)."""
+    return {"tiny": 8, "lofar": 48, "sweep": 48, "ska": 128, "paper": 55}[name]
+
+
 def make_workload(name: str, device="cpu", *, n_baselines: Optional[int] = None,
                   n_time: Optional[int] = None, subgrid_size: Optional[int] = None,
                   max_timesteps: Optional[int] = None, max_channels: Optional[int] = None,
                   aterm_interval: Optional[int] = None, flags: Optional[int] = None,
                   identity_a: bool = False, seed_offset: int = 0,
-                  baseline_offset: int = 0) -> Workload:
+                  baseline_offset: int = 0, baseline_stride: int = 1) -> Workload:
     """Build one of BASELINE.json's workloads ("tiny", "lofar", "ska", "sweep").
 
     Optional overrides shrink it (first ``n_baselines`` baselines starting at
-    ``baseline_offset``, first ``n_time`` timesteps) or change the plan
+    ``baseline_offset``, every ``baseline_stride``-th of those, first ``n_time`` timesteps) or change the plan
     parameters (the sweep of config 4).  ``seed_offset`` gives another
     realisation of the same shape (used to hand every rank of a weak-scaling
     run its own data).
@@ -291,6 +296,8 @@ def make_workload(name: str, device="cpu", *, n_baselines: Optional[int] = None,
     if n_baselines is not None or baseline_offset:
         end = len(bl) if n_baselines is None else baseline_offset + n_baselines
         bl = bl[baseline_offset:end]
+    if baseline_stride > 1:
+        bl = np.ascontiguousarray(bl[::baseline_stride])
     T = c["T"] if n_time is None else n_time
     uvw_np = earth_rotation_uvw(enu, bl, c["lat"], c["dec"], -30.0, c["dt"], T)
     freqs = c["f0"] + c["df"] * np.arange(c["C"], dtype=np.float64)
