@@ -202,6 +202,21 @@ int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *cu
  * {16, 24, 32, 48}, L >= N even.  Asynchronous on cuda_stream; allocates (and frees, stream-ordered) 32 L N bytes. */
 int idg_image_taper(const float *taper_dev, int32_t N, float *cbar_dev, int32_t L, void *cuda_stream);
 
+/* ---- optimal taper (offline input of the hot path) ----------------------------------
+ * Section 4.3, Appendix A: the taper c[i][j] = a_i a_j (Eq. 30) whose effective
+ * window has the least side-lobe energy, averaged over the sample shifts |s| <= (N - beta + 1)/2 a kernel budget of
+ * beta pixels allows: a = eigenvector of the smallest eigenvalue of R-bar = Q-bar (.) S-bar (Eq. 36-37, A.3-A.8),
+ * minimised over a_1 .. a_{N-1} with a_0 = 0 so that the window is symmetric about the centre pixel N/2 (reading R16;
+ * this reproduces Table 1).  beta plays the role of idg_plan_params.kernel_size.
+ *   taper_dev     [N][N] float32, device, written: a_i a_j scaled to 1 at the centre pixel
+ *   a_host        [N] float64, host, optional: the coefficients (a_host[N/2] = 1, a_host[0] = 0)
+ *   epsilon_host  optional: the aliasing level sqrt(lambda_min) of Table 1; FP64 resolves it down to ~1e-7, below
+ *                 that the window is still near-optimal but the value returned is not reliable
+ * N even, 4 <= N <= 64 (every subgrid size of the library and every column of Table 1); 1 <= beta < N.
+ * Runs one FP64 CTA on cuda_stream and synchronises it.  Errors: IDG_ERR_INVALID_ARG, IDG_ERR_CUDA. */
+int idg_taper_optimal(int32_t N, double beta, float *taper_dev, double *a_host, double *epsilon_host,
+                      void *cuda_stream);
+
 /* ---- scalar variant: one polarisation ------------------------------------------
  * The method as the paper derives it before the 2x2 substitution (Eq. 1-25);
  * "Stokes I only" is how the classical gridder is timed in PAPER.md:481.  Complex gains g (Eq. 2):

@@ -27,7 +27,7 @@ EXPORTS = (
     "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
     "idg_adder", "idg_splitter", "idg_splitter_ifft", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
-    "idg_image_divide", "idg_image_taper", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
+    "idg_image_divide", "idg_image_taper", "idg_taper_optimal", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
 
 
 class IdgError(RuntimeError):
@@ -357,6 +357,18 @@ def idg_image_taper(taper, L: int, stream=None) -> torch.Tensor:
     _check(lib().idg_image_taper(_dev(taper, _F32, "taper"), ctypes.c_int32(N), _dev(out, _F32, "cbar"),
                                  ctypes.c_int32(int(L)), _stream(stream)), "idg_image_taper")
     return out
+
+
+def idg_taper_optimal(N: int, beta: float, device="cuda", stream=None):
+    """Optimal IDG taper (NEXT-2, section 4.3 / Appendix A): -> (taper [N][N] float32 on `device`, a [N] float64
+    numpy, epsilon)."""
+    taper = torch.empty((int(N), int(N)), dtype=_F32, device=device)
+    a = np.zeros(int(N), dtype=np.float64)
+    eps = ctypes.c_double()
+    _check(lib().idg_taper_optimal(ctypes.c_int32(int(N)), ctypes.c_double(float(beta)), _dev(taper, _F32, "taper"),
+                                   ctypes.c_void_p(a.ctypes.data), ctypes.byref(eps), _stream(stream)),
+           "idg_taper_optimal")
+    return taper, a, float(eps.value)
 
 
 def _scalar_check(plan: Plan, uvw, vis, gains, taper, grid=None, subgrids=None):
