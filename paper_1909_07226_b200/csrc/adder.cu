@@ -5,14 +5,17 @@
 // Splitter (Alg. 2): V_p[pol][b][a] = grid[pol][y0+b][x0+a].
 //
 // Subgrids overlap ("subgrids may overlap"), heavily near the uv origin.  Instead
-// of one atomic per subgrid pixel, the plan buckets the subgrids by the 128 x 8 grid tiles they
-// touch (stable in the subgrid index; wide tiles so that a subgrid row is rarely split between two
-// work items -- a split 32-byte sector is fetched from HBM twice).  One work item = one tile and
-// up to kAdderChunk of its subgrids: the CTA sums their overlapping parts into a shared-memory
-// copy of the tile in plan order and adds the tile to the grid once, with one vector reduction
-// (red.global.add.v2.f32) per touched pixel.  Every subgrid element is read exactly once; the
-// grid sees one reduction per (work item, pixel) instead of one per (subgrid, pixel).  Long lists
-// (the uv core) are split over several work items so no CTA becomes the tail.
+// of one atomic per subgrid pixel, the plan buckets the subgrids by grid tiles: a subgrid belongs
+// to the 128-pixel tile COLUMN its x0 falls in and to every 8-row band it overlaps (stable in the
+// subgrid index).  One work item = one tile and up to kAdderChunk of its subgrids: the CTA sums
+// their rows into a shared-memory accumulator of 8 rows x (128 + N) pixels -- wide enough for a
+// subgrid that starts in the last column of the tile -- in plan order and adds it to the grid
+// once, with one vector reduction (red.global.add.v2.f32) per touched pixel.  Every subgrid row
+// is read exactly once and WHOLE (256 contiguous, aligned bytes at N = 32: no sector or DRAM
+// burst is fetched twice, which rows split between two tile columns cost the first version); the
+// grid sees one reduction per (work item, pixel) instead of one per (subgrid, pixel); the N
+// columns two neighbouring tiles share receive reductions from both.  Long lists (the uv core)
+// are split over several work items so no CTA becomes the tail.
 #include <algorithm>
 
 #include "common.cuh"
@@ -32,9 +35,9 @@ adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
   // the rows w / NPOL + (8 / NPOL) k of the tile: every (pol, row) slot has exactly one writer, so the
   // accumulation needs neither atomics nor barriers, and a warp always reads whole subgrid rows
   // (N consecutive float2: 256 B at N = 32), one lane per pixel.
-  constexpr int TX = kAdderTileX, TY = kAdderTileY, RSTEP = 8 / NPOL, ROWS = TY / RSTEP;
+  constexpr int TX = kAdderTileX + N, TY = kAdderTileY, RSTEP = 8 / NPOL, ROWS = TY / RSTEP;
   constexpr int PASSES = (N + 31) / 32;            // N = 48: a row takes two passes of 32 lanes
-  __shared__ float2 tile[NPOL][TY][TX];
+  __shared__ float2 tile[NPOL][TY][TX];            // 128 + N columns: x0 - tile_x <= 127, so x0 - tile_x + N - 1 < TX
   const AdderItem it = items[blockIdx.x];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int q = warp % NPOL, r0 = warp / NPOL;
@@ -59,8 +62,8 @@ adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
         ok[j][k] = have && sy >= 0 && sy < N;
 #pragma unroll
         for (int p = 0; p < PASSES; ++p) {
-          const int sx = lane + 32 * p, x = tx0[j] + sx;    // lanes outside the tile do not load
-          v[j][k][p] = (ok[j][k] && sx < N && x >= 0 && x < TX) ? __ldg(&sg[sy * N + sx]) : make_float2(0.f, 0.f);
+          const int sx = lane + 32 * p;
+          v[j][k][p] = (ok[j][k] && sx < N) ? __ldg(&sg[sy * N + sx]) : make_float2(0.f, 0.f);
         }
       }
     }
@@ -72,7 +75,7 @@ adder_kernel(const AdderItem *__restrict__ items, const int4 *__restrict__ list,
 #pragma unroll
           for (int p = 0; p < PASSES; ++p) {
             const int sx = lane + 32 * p, x = tx0[j] + sx;
-            if (sx < N && x >= 0 && x < TX) {
+            if (sx < N) {
               float2 a = tile[q][r0 + RSTEP * k][x];
               a.x += v[j][k][p].x; a.y += v[j][k][p].y;
               tile[q][r0 + RSTEP * k][x] = a;

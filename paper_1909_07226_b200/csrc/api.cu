@@ -30,15 +30,15 @@ static int check_params(const idg_plan_params *p) {
   return IDG_OK;
 }
 
-// Bucket the subgrids by the 128 x 8 grid tiles they overlap (stable counting sort in p) and cut every
-// tile's list into work items of at most kAdderChunk subgrids.
+// Bucket the subgrids by grid tiles (stable counting sort in p): tile column = the 128-pixel column x0 falls in,
+// tile rows = every 8-row band the subgrid overlaps; cut every tile's list into work items of at most kAdderChunk
+// subgrids.
 static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
   const int N = pl->prm.subgrid_size, L = pl->prm.grid_size, TX = kAdderTileX, TY = kAdderTileY;
   const int ntx = (L + TX - 1) / TX, nty = (L + TY - 1) / TY;
   std::vector<int64_t> offs((size_t)ntx * nty + 1, 0);
   for (const auto &m : pl->meta_host)
-    for (int ty = m.y0 / TY; ty <= (m.y0 + N - 1) / TY; ++ty)
-      for (int tx = m.x0 / TX; tx <= (m.x0 + N - 1) / TX; ++tx) ++offs[(size_t)ty * ntx + tx + 1];
+    for (int ty = m.y0 / TY; ty <= (m.y0 + N - 1) / TY; ++ty) ++offs[(size_t)ty * ntx + m.x0 / TX + 1];
   for (size_t i = 1; i < offs.size(); ++i) offs[i] += offs[i - 1];
   const int64_t total = offs.back();
   if (total > (int64_t)INT32_MAX) return IDG_ERR_INVALID_ARG;   // AdderItem ranges are int32
@@ -47,8 +47,7 @@ static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
   for (int64_t p = 0; p < pl->P; ++p) {
     const auto &m = pl->meta_host[(size_t)p];
     for (int ty = m.y0 / TY; ty <= (m.y0 + N - 1) / TY; ++ty)
-      for (int tx = m.x0 / TX; tx <= (m.x0 + N - 1) / TX; ++tx)
-        list[(size_t)cur[(size_t)ty * ntx + tx]++] = (int32_t)p;
+      list[(size_t)cur[(size_t)ty * ntx + m.x0 / TX]++] = (int32_t)p;
   }
   // work items of at most `chunk` subgrids: kAdderChunk when there is plenty of work, shorter lists on small
   // plans so that the items still fill the GPU (a few per resident CTA slot)
@@ -59,11 +58,11 @@ static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
       const int64_t b = offs[(size_t)ty * ntx + tx], e = offs[(size_t)ty * ntx + tx + 1];
       for (int64_t s = b; s < e; s += chunk) {
         const int64_t se = std::min<int64_t>(e, s + chunk);
-        int lo = TX, hi = 0;
+        int lo = TX + N, hi = 0;          // accumulator columns this item's subgrids cover (of 128 + N)
         for (int64_t i = s; i < se; ++i) {
           const int x0 = pl->meta_host[(size_t)list[(size_t)i]].x0 - tx * TX;
-          lo = std::min(lo, std::max(0, x0));
-          hi = std::max(hi, std::min(TX, x0 + N));
+          lo = std::min(lo, x0);
+          hi = std::max(hi, x0 + N);
         }
         items.push_back(AdderItem{tx * TX, ty * TY, (int32_t)s, (int32_t)se, lo, hi});
       }

@@ -12,14 +12,14 @@
 namespace idg {
 
 constexpr double kSpeedOfLight = 299792458.0;
-constexpr int kAdderTileX = 128;     // grid tile owned by one adder work item: 128 (x) by 8 (y) pixels.  Wide tiles
-constexpr int kAdderTileY = 8;       // keep the subgrid rows (256 B at N = 32) whole: few split 32-byte sectors
+constexpr int kAdderTileX = 128;     // adder work item: the subgrids whose x0 lies in a 128-pixel column, one 8-row
+constexpr int kAdderTileY = 8;       // band of the grid at a time (accumulator 8 rows x (128 + N) pixels)
 constexpr int kAdderChunk = 64;      // max subgrids accumulated by one work item
 
 struct AdderItem {                    // one unit of adder work: a grid tile and a slice of its list
   int32_t tile_x, tile_y;             // tile origin on the grid (pixels)
   int32_t begin, end;                 // range in adder_list
-  int32_t x_lo, x_hi;                 // tile-local x extent its subgrids cover (zeroed / flushed range)
+  int32_t x_lo, x_hi;                 // accumulator columns its subgrids cover (zeroed / flushed range), 0 .. 128 + N
 };
 
 }  // namespace idg
