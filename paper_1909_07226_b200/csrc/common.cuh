@@ -12,7 +12,7 @@
 namespace idg {
 
 constexpr double kSpeedOfLight = 299792458.0;
-constexpr int kAdderTileX = 128;     // adder work item: the subgrids whose x0 lies in a 128-pixel column, one 8-row
+constexpr int kAdderTileX = 96;  // adder work item: the subgrids whose x0 lies in a 128-pixel column, one 8-row
 constexpr int kAdderTileY = 8;       // band of the grid at a time (accumulator 8 rows x (128 + N) pixels)
 constexpr int kAdderChunk = 64;      // max subgrids accumulated by one work item
 
