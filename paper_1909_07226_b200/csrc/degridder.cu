@@ -36,10 +36,7 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
   // (re XX, re XY, re YX, re YY), (im ...) -- one FFMA2 updates two polarisations
   __shared__ float4 s_pix[CH * 2];
   __shared__ float4 s_lmn[CH];       // l, m, n', unused
-  // partial sums of the SPLIT reduction: NT CPT 8 floats at most; the pixel staging area is reused when it is
-  // large enough (N >= 24), N = 16 gets its own
-  constexpr bool kOwnRed = SPLIT && (CH * 8 < NT * CPT * 8);
-  __shared__ float s_red_own[kOwnRed ? NT * CPT * 8 : 1];
+  static_assert(CH * 8 >= NT * 8, "the SPLIT reduction reuses the pixel staging area, [NT][8] floats");
 
   const int tid = threadIdx.x;
   const idg_subgrid_meta m = meta[blockIdx.x];
@@ -53,8 +50,10 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
   const double w0 = w_step > 0.0 ? ((double)m.w_index + 0.5) * w_step : 0.0;
   const double k_mid = 0.5 * (freqs[m.chan_begin] + freqs[m.chan_begin + n_chan - 1]) * inv_c0;
 
-  const int groups = (n_chan + CPT - 1) / CPT;       // channel groups per timestep
-  const int n_items = n_time * groups;
+  // ONECHAN (single-channel plans): a thread owns CPT consecutive TIMESTEPS of the one channel instead of CPT
+  // channels of one timestep, so that the three shared-memory reads per pixel still serve CPT visibilities
+  const int groups = ONECHAN ? 1 : (n_chan + CPT - 1) / CPT;       // channel groups per timestep
+  const int n_items = ONECHAN ? (n_time + CPT - 1) / CPT : n_time * groups;
   // IDG_PLAN_SPAN_ATERMS (NEXT-4, per-sample c_pk: Alg. 2): the block is walked slot by slot; the
   // corrected pixels are staged with the slot's Jones matrices and only the threads whose timestep lies in
   // that slot accumulate.  Without the flag there is one slot, m.aterm_slot.
@@ -70,18 +69,28 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
   for (int item0 = 0; item0 < n_items; item0 += NT) {
     const int item = SPLIT ? tid - grp * n_items : item0 + tid;
     const bool active = SPLIT ? grp < G : item < n_items;
-    const int tl = active ? item / groups : 0;
-    const int cg = active ? (item - tl * groups) * CPT : 0;
+    const int tl = active ? (ONECHAN ? item * CPT : item / groups) : 0;
+    const int cg = (active && !ONECHAN) ? (item - tl * groups) * CPT : 0;
     const float *p = uvw + ((size_t)m.baseline * T + (m.time_begin + tl)) * 3;
     const float u = p[0], v = p[1], w = p[2];
     const float bu = (float)(two_pi * ((double)u * k_mid - u0));
     const float bv = (float)(two_pi * ((double)v * k_mid - v0));
     const float bw = (float)(two_pi * ((double)w * k_mid - w0));
     float kd[CPT];
+    constexpr int NB = ONECHAN ? CPT : 1;           // ONECHAN: the phase coefficients of each of the CPT timesteps
+    float bus[NB], bvs[NB], bws[NB];
 #pragma unroll
     for (int c = 0; c < CPT; ++c) {
-      const int cc = min(cg + c, n_chan - 1);
-      kd[c] = (float)(two_pi * (freqs[m.chan_begin + cc] * inv_c0 - k_mid));
+      if (ONECHAN) {
+        const float *pc = uvw + ((size_t)m.baseline * T + (m.time_begin + min(tl + c, n_time - 1))) * 3;
+        bus[c] = (float)(two_pi * ((double)pc[0] * k_mid - u0));
+        bvs[c] = (float)(two_pi * ((double)pc[1] * k_mid - v0));
+        bws[c] = (float)(two_pi * ((double)pc[2] * k_mid - w0));
+        kd[c] = 0.f;
+      } else {
+        const int cc = min(cg + c, n_chan - 1);
+        kd[c] = (float)(two_pi * (freqs[m.chan_begin + cc] * inv_c0 - k_mid));
+      }
     }
     float2 re01[CPT], re23[CPT], im01[CPT], im23[CPT];
 #pragma unroll
@@ -99,8 +108,8 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
       // stage Dg = A1 (taper Ip) A2^H and the pixel coordinates for this chunk
       for (int i = tid; i < npx; i += NT) {
         const int pix = pix0 + i;
-        if (CPT >= 8 && !(N == 16 && NT == 256)) {
-          s_lmn[i] = __ldg(&lmn[pix]);       // the plan's table
+        if ((CPT >= 8 || SPLIT || ONECHAN) && !(N == 16 && NT == 256)) {
+          s_lmn[i] = __ldg(&lmn[pix]);       // the plan's table (always for short blocks: their staging phase counts)
         } else {
           // measured: with 1-4 channels per thread (and in the N = 16, 256-thread instance) the kernel is 2-4 % faster
           // when the staging phase computes the direction cosines (same values as the table: R1, R2 in FP64,
@@ -141,11 +150,12 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
           const float4 qr = s_pix[2 * i], qi = s_pix[2 * i + 1];
           // single-channel plans: kd = 0 exactly, the phase is `base` alone
           const float pidx = ONECHAN ? 0.f : fmaf(u, c3.x, fmaf(v, c3.y, w * c3.z));
-          const float base = fmaf(bu, c3.x, fmaf(bv, c3.y, bw * c3.z));
+          const float base = ONECHAN ? 0.f : fmaf(bu, c3.x, fmaf(bv, c3.y, bw * c3.z));
 #pragma unroll
           for (int c = 0; c < CPT; ++c) {
             float s, co;
-            __sincosf(ONECHAN ? base : fmaf(pidx, kd[c], base), &s, &co);
+            __sincosf(ONECHAN ? fmaf(bus[ONECHAN ? c : 0], c3.x, fmaf(bvs[ONECHAN ? c : 0], c3.y, bws[ONECHAN ? c : 0] * c3.z))
+                              : fmaf(pidx, kd[c], base), &s, &co);
             const float ns = -s;
             // (re + i im) += (qr + i qi)(co - i s): the conjugate phasor of the gridder
             re01[c] = ffma2(dlo2(qr), dbc2(co), re01[c]); re01[c] = ffma2(dlo2(qi), dbc2(s), re01[c]);
@@ -158,24 +168,57 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
     }
     }
     if (SPLIT && G > 1) {
-      float *red = kOwnRed ? s_red_own : reinterpret_cast<float *>(s_pix);   // [G - 1][n_items][CPT][8]
-      __syncthreads();
-      if (active && grp > 0) {
-        float *r = red + ((size_t)(grp - 1) * n_items + item) * (CPT * 8);
-#pragma unroll
-        for (int c = 0; c < CPT; ++c) {
-          r[8 * c + 0] = re01[c].x; r[8 * c + 1] = re01[c].y; r[8 * c + 2] = re23[c].x; r[8 * c + 3] = re23[c].y;
-          r[8 * c + 4] = im01[c].x; r[8 * c + 5] = im01[c].y; r[8 * c + 6] = im23[c].x; r[8 * c + 7] = im23[c].y;
-        }
-      }
-      __syncthreads();
-      if (active && grp == 0) {
-        for (int g = 1; g < G; ++g) {
-          const float *r = red + ((size_t)(g - 1) * n_items + item) * (CPT * 8);
+      // partial sums of the pixel groups through the pixel staging area
+      constexpr int SPR = (CH / NT) >= CPT ? CPT : (CH / NT);      // channel slots that fit per round
+      static_assert(SPR >= 1, "the staging area must hold one slot per thread");
+      float *red = reinterpret_cast<float *>(s_pix);
+      if (SPR == CPT) {
+        // N >= 32: all slots at once, [G - 1][n_items][CPT][8].  (A bank-conflict-free [slot][component][thread]
+        // layout measured 1 % SLOWER on the SKA-like plan: the phase is a few hundred cycles of a 120 k-cycle CTA and
+        // the change moved the register allocation of the main loop.)
+        __syncthreads();
+        if (active && grp > 0) {
+          float *r = red + ((size_t)(grp - 1) * n_items + item) * (CPT * 8);
 #pragma unroll
           for (int c = 0; c < CPT; ++c) {
-            re01[c].x += r[8 * c + 0]; re01[c].y += r[8 * c + 1]; re23[c].x += r[8 * c + 2]; re23[c].y += r[8 * c + 3];
-            im01[c].x += r[8 * c + 4]; im01[c].y += r[8 * c + 5]; im23[c].x += r[8 * c + 6]; im23[c].y += r[8 * c + 7];
+            r[8 * c + 0] = re01[c].x; r[8 * c + 1] = re01[c].y; r[8 * c + 2] = re23[c].x; r[8 * c + 3] = re23[c].y;
+            r[8 * c + 4] = im01[c].x; r[8 * c + 5] = im01[c].y; r[8 * c + 6] = im23[c].x; r[8 * c + 7] = im23[c].y;
+          }
+        }
+        __syncthreads();
+        if (active && grp == 0) {
+          for (int g = 1; g < G; ++g) {
+            const float *r = red + ((size_t)(g - 1) * n_items + item) * (CPT * 8);
+#pragma unroll
+            for (int c = 0; c < CPT; ++c) {
+              re01[c].x += r[8 * c + 0]; re01[c].y += r[8 * c + 1]; re23[c].x += r[8 * c + 2]; re23[c].y += r[8 * c + 3];
+              im01[c].x += r[8 * c + 4]; im01[c].y += r[8 * c + 5]; im23[c].x += r[8 * c + 6]; im23[c].y += r[8 * c + 7];
+            }
+          }
+        }
+      } else {
+        // N < 32: rounds of SPR slots, [slot][component][thread] (consecutive threads, consecutive banks)
+#pragma unroll
+        for (int c0 = 0; c0 < CPT; c0 += SPR) {
+          __syncthreads();
+          if (active && grp > 0) {
+#pragma unroll
+            for (int c = c0; c < c0 + SPR && c < CPT; ++c) {
+              float *rc = red + (size_t)(c - c0) * 8 * NT + tid;            // tid = grp * n_items + item
+              rc[0 * NT] = re01[c].x; rc[1 * NT] = re01[c].y; rc[2 * NT] = re23[c].x; rc[3 * NT] = re23[c].y;
+              rc[4 * NT] = im01[c].x; rc[5 * NT] = im01[c].y; rc[6 * NT] = im23[c].x; rc[7 * NT] = im23[c].y;
+            }
+          }
+          __syncthreads();
+          if (active && grp == 0) {
+            for (int g = 1; g < G; ++g) {
+#pragma unroll
+              for (int c = c0; c < c0 + SPR && c < CPT; ++c) {
+                const float *rc = red + (size_t)(c - c0) * 8 * NT + g * n_items + item;
+                re01[c].x += rc[0 * NT]; re01[c].y += rc[1 * NT]; re23[c].x += rc[2 * NT]; re23[c].y += rc[3 * NT];
+                im01[c].x += rc[4 * NT]; im01[c].y += rc[5 * NT]; im23[c].x += rc[6 * NT]; im23[c].y += rc[7 * NT];
+              }
+            }
           }
         }
       }
@@ -184,23 +227,23 @@ degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restr
       float4 *o = vis_out + (((size_t)m.baseline * T + (m.time_begin + tl)) * C + m.chan_begin + cg) * 2;
 #pragma unroll
       for (int c = 0; c < CPT; ++c) {
-        if (cg + c < n_chan) {
-          o[2 * c] = make_float4(re01[c].x, im01[c].x, re01[c].y, im01[c].y);
-          o[2 * c + 1] = make_float4(re23[c].x, im23[c].x, re23[c].y, im23[c].y);
+        if (ONECHAN ? tl + c < n_time : cg + c < n_chan) {
+          float4 *oc = ONECHAN ? o + (size_t)c * C * 2 : o + 2 * c;      // next timestep / next channel
+          oc[0] = make_float4(re01[c].x, im01[c].x, re01[c].y, im01[c].y);
+          oc[1] = make_float4(re23[c].x, im23[c].x, re23[c].y, im23[c].y);
         }
       }
     }
   }
 }
 
-template <int N, int NT, int CPT, bool SPLIT = false>
+template <int N, int NT, int CPT, bool SPLIT = false, bool ONE = false>
 static int launch_k(const idg_plan *plan, const float *uvw, const float2 *subgrids,
                     const float2 *aterms, const float *taper, float2 *vis_out, cudaStream_t stream,
                     int64_t p0, int64_t np) {
   const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
-  const bool one = CPT == 1 && !span && plan->max_n_chan == 1;
   auto kern = span ? degridder_kernel<N, NT, CPT, true, SPLIT>
-                   : (one ? degridder_kernel<N, NT, (CPT == 1 ? 1 : CPT), false, SPLIT, CPT == 1>
+                   : (ONE ? degridder_kernel<N, NT, CPT, false, SPLIT, ONE>
                           : degridder_kernel<N, NT, CPT, false, SPLIT>);
   kern<<<(unsigned)np, NT, 0, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, plan->lmn_dev, subgrids + (size_t)p0 * 4 * N * N,
@@ -232,13 +275,23 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
                     int64_t p0, int64_t np) {
   // threads own (timestep, CPT channels); pick CPT and the CTA size from the plan's largest block
   const int mc = plan->max_n_chan;
+  // single-channel plans: kd = 0 and the phase is `base` alone; threads own four consecutive timesteps (the pixel
+  // reads from shared memory are shared by the four), the pixels are split over thread groups when the block is short
+  if (mc == 1 && (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) == 0) {
+    if (plan->max_n_time < 8)
+      return launch_k<N, 128, 1, true, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    const int items4 = (plan->max_n_time + 3) / 4;
+    if (items4 <= 64) return launch_k<N, 128, 4, true, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    if (items4 <= 128) return launch_k<N, 128, 4, false, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    return launch_k<N, 256, 4, false, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+  }
   // more channels per thread amortise the per-pixel shared-memory reads and phase set-up, as long as the
   // largest block still fills a 128-thread CTA
   int cpt = mc >= 4 ? 4 : (mc >= 2 ? 2 : 1);
   const int items8 = plan->max_n_time * ((mc + 7) / 8);
   // 8 channels per thread when that still fills a 128-thread CTA, or (N >= 32) half of one: then two thread groups
   // share the pixels (SPLIT below)
-  if (mc >= 8 && (items8 >= 128 || (N >= 32 && items8 >= 32 && items8 <= 64))) cpt = 8;
+  if (mc >= 8 && (items8 >= 128 || (N >= 24 && items8 >= 16 && items8 <= 64) || (N >= 32 && items8 >= 32 && items8 <= 64))) cpt = 8;
   // plans that mix channel-group sizes (a 20-channel band cut into 16 + 4) and would idle more than 5 % of the
   // 8-channel slots: two launches, 8 channels per thread on the subgrids that fill them, 4 on the rest
   if (cpt == 8 && items8 >= 128 && plan->dg_waste[3] > 0.05f && plan->dg_waste[2] <= 0.05f &&
@@ -254,8 +307,8 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
   while (cpt > 1 && plan->dg_waste[cpt == 8 ? 3 : (cpt == 4 ? 2 : 1)] > 0.05f) cpt /= 2;
   const int items = plan->max_n_time * ((mc + cpt - 1) / cpt);
   const bool small = items <= 128;
-  if (N >= 32 && items <= 64 && cpt == 8)
-    return launch_k<(N >= 32 ? N : 32), 128, 8, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+  if (items <= 64 && cpt == 8)
+    return launch_k<N, 128, 8, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
   if (items <= 64 && cpt <= 4 && N >= 24) {   // short blocks: split the pixels over thread groups (measured: no gain at N = 16)
     if (cpt == 4) return launch_k<N, 128, 4, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     if (cpt == 2) return launch_k<N, 128, 2, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);

@@ -440,7 +440,12 @@ def test_ska_slice_sampled():
                                                  # long blocks: many staging batches per CTA; N = 24 above 4096 visibilities per
                                                  # block takes the 64-thread gridder instance; (32, 16, 512, 32) the degridder
                                                  # with 8 channels per thread and two pixel groups
-                                                 (16, 64, 512, 128), (24, 16, 256, 256), (24, 16, 512, 512), (32, 16, 512, 32)])
+                                                 (16, 64, 512, 128), (24, 16, 256, 256), (24, 16, 512, 512), (32, 16, 512, 32),
+                                                 # round 2: single-channel plans tile four timesteps per thread (split and
+                                                 # unsplit instances); 8 channels per thread with eight pixel groups and the
+                                                 # reduction in rounds (N = 24) or at once (N = 48)
+                                                 (16, 1, 512, 512), (24, 1, 128, 256), (48, 1, 32, 512), (24, 16, 512, 8), (48, 16, 512, 8),
+                                                 (16, 16, 512, 8)])
 def test_sweep_corners_sampled(N, max_c, max_t, a_int):
     w = synth.make_workload("sweep", n_baselines=12, n_time=512, subgrid_size=N, max_channels=max_c,
                             max_timesteps=max_t, aterm_interval=a_int)
