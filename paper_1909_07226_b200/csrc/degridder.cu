@@ -23,7 +23,7 @@ __device__ __forceinline__ float2 dhi2(float4 v) { return make_float2(v.z, v.w);
 // FILT selects the subgrids a launch works on (plans that mix channel-group sizes are degridded in two launches):
 // 0 all, 1 only those with n_chan a multiple of 8, 2 only the others.
 template <int N, int NT, int CPT, bool SPAN, bool SPLIT, bool ONECHAN = false, int FILT = 0>
-__global__ void __launch_bounds__(NT, NT == 128 ? 4 : 2)
+__global__ void __launch_bounds__(NT, NT == 128 ? 4 : (NT == 64 ? 8 : (NT == 32 ? 16 : 2)))
 degridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                  const double *__restrict__ freqs, const float4 *__restrict__ lmn,
                  const float2 *__restrict__ subgrids,
@@ -281,6 +281,12 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
     if (plan->max_n_time < 8)
       return launch_k<N, 128, 1, true, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     const int items4 = (plan->max_n_time + 3) / 4;
+    // N = 16: a block of up to 32 items is one warp's work; single-warp CTAs (16 per SM, no idle threads, barriers
+    // that cost nothing) measured 0.63 of the roofline against 0.58 for 128 threads in four pixel groups
+    if constexpr (N == 16)
+      if (items4 <= 32) return launch_k<N, 32, 4, false, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+    if constexpr (N == 24)      // two warps, two pixel groups: 0.61 against 0.60 (128 threads) and 0.55 (one warp)
+      if (items4 <= 32) return launch_k<N, 64, 4, true, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     if (items4 <= 64) return launch_k<N, 128, 4, true, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     if (items4 <= 128) return launch_k<N, 128, 4, false, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     return launch_k<N, 256, 4, false, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
@@ -309,6 +315,8 @@ static int launch_n(const idg_plan *plan, const float *uvw, const float2 *subgri
   const bool small = items <= 128;
   if (items <= 64 && cpt == 8)
     return launch_k<N, 128, 8, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
+  if constexpr (N == 16)      // single-warp CTAs for blocks of at most 32 (timestep, 4 channels) items, as above
+    if (items <= 32 && cpt == 4) return launch_k<N, 32, 4>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
   if (items <= 64 && cpt <= 4 && N >= 24) {   // short blocks: split the pixels over thread groups (measured: no gain at N = 16)
     if (cpt == 4) return launch_k<N, 128, 4, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     if (cpt == 2) return launch_k<N, 128, 2, true>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);

@@ -33,7 +33,7 @@ __device__ __forceinline__ float2 bc2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
 __device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
 
-template <int N, int NT, int PPT, int MINB, int VB, int TB, bool SPAN, bool ONECHAN>
+template <int N, int NT, int PPT, int MINB, int VB, int TB, bool SPAN, bool ONECHAN, int SPL = 1>
 __global__ void __launch_bounds__(NT, MINB)
 gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                const double *__restrict__ freqs, const float4 *__restrict__ lmn, const float4 *__restrict__ vis,
@@ -41,12 +41,15 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
                float2 *__restrict__ subgrids, int32_t T, int32_t C, int32_t n_stations,
                int32_t L, double image_size, double w_step, int32_t aterm_interval) {
   constexpr int vis_batch = VB, time_batch = TB;
-  static_assert(NT * PPT == N * N, "pixels must tile the CTA exactly");
+  // SPL CTAs share one subgrid (blockIdx.y = which part of its pixels): at N = 48 two 192-thread CTAs per subgrid
+  // run two to an SM, so that one's staging phase and epilogue hide behind the other's visibility loop
+  static_assert(NT * PPT * SPL == N * N, "pixels must tile the CTAs exactly");
+  const int pix_base = SPL > 1 ? blockIdx.y * (NT * PPT) : 0;
   extern __shared__ float4 g_smem[];
   float4 *s_vis = g_smem;                  // [vis_batch][2]: (re XX, re XY, re YX, re YY), (im ...)
   float4 *s_t = s_vis + vis_batch * 2;     // [time_batch][2]: (u, v, w, -), (bu, bv, bw, -)
-  float4 *s_lmn = s_t + time_batch * 2;    // [N*N]: (l, m, n', -) per pixel
-  float *s_kd = reinterpret_cast<float *>(s_lmn + N * N);   // [kMaxChan]
+  float4 *s_lmn = s_t + time_batch * 2;    // [NT*PPT]: (l, m, n', -) per pixel of this CTA
+  float *s_kd = reinterpret_cast<float *>(s_lmn + NT * PPT);   // [kMaxChan]
 
   const int tid = threadIdx.x;
   const idg_subgrid_meta m = meta[blockIdx.x];
@@ -66,15 +69,15 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
   // measured 3-4 % slower with the table load than with the FP64 evaluation and keep the latter (same values).
 #pragma unroll
   for (int k = 0; k < PPT; ++k) {
-    const int pix = tid + k * NT;
+    const int pix = pix_base + tid + k * NT;
     if (N != 24) {
-      s_lmn[pix] = __ldg(&lmn[pix]);
+      s_lmn[tid + k * NT] = __ldg(&lmn[pix]);
     } else {
       const int y = pix / N, x = pix - y * N;
       const double l = (double)(x - N / 2) * image_size / (double)N;
       const double mm = (double)(y - N / 2) * image_size / (double)N;
       const double r2 = l * l + mm * mm;
-      s_lmn[pix] = make_float4((float)l, (float)mm, (float)(-r2 / (1.0 + sqrt(1.0 - r2))), 0.f);
+      s_lmn[tid + k * NT] = make_float4((float)l, (float)mm, (float)(-r2 / (1.0 + sqrt(1.0 - r2))), 0.f);
     }
   }
 
@@ -91,7 +94,7 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
     float2 *out = subgrids + (size_t)blockIdx.x * 4 * N * N;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
-      const int pix = tid + k * NT;
+      const int pix = pix_base + tid + k * NT;
       const float4 a01 = __ldg(&aterms[(a1_off + pix) * 2]), a23 = __ldg(&aterms[(a1_off + pix) * 2 + 1]);
       const float4 b01 = __ldg(&aterms[(a2_off + pix) * 2]), b23 = __ldg(&aterms[(a2_off + pix) * 2 + 1]);
       const float tp = __ldg(&taper[pix]);
@@ -209,20 +212,20 @@ gridder_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restric
 // VB visibilities and TB timesteps are staged per batch.  Every batch costs the CTA two barriers, at which its
 // faster warps idle; larger batches measured +2.5 % (N = 32, 48) and up to +10 % (N = 24, blocks of 2048-4096
 // visibilities) over 256-visibility batches.  Single-channel plans keep 256 timesteps per batch.
-template <int N, int NT, int PPT, int MINB, int VB, int TB>
+template <int N, int NT, int PPT, int MINB, int VB, int TB, int SPL = 1>
 static int launch_n(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
                     const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
   const bool span = (plan->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
   // single-channel plans without the span flag take the ONECHAN instance
   const bool one = !span && plan->max_n_chan == 1;
-  constexpr size_t smem_one = sizeof(float4) * (256 * 4 + N * N) + sizeof(float) * kMaxChan;
-  constexpr size_t smem_any = sizeof(float4) * ((size_t)VB * 2 + (size_t)TB * 2 + N * N) + sizeof(float) * kMaxChan;
+  constexpr size_t smem_one = sizeof(float4) * (256 * 4 + NT * PPT) + sizeof(float) * kMaxChan;
+  constexpr size_t smem_any = sizeof(float4) * ((size_t)VB * 2 + (size_t)TB * 2 + NT * PPT) + sizeof(float) * kMaxChan;
   const size_t smem = one ? smem_one : smem_any;
-  auto kern = span ? gridder_kernel<N, NT, PPT, MINB, VB, TB, true, false>
-                   : (one ? gridder_kernel<N, NT, PPT, MINB, 256, 256, false, true>
-                          : gridder_kernel<N, NT, PPT, MINB, VB, TB, false, false>);
+  auto kern = span ? gridder_kernel<N, NT, PPT, MINB, VB, TB, true, false, SPL>
+                   : (one ? gridder_kernel<N, NT, PPT, MINB, 256, 256, false, true, SPL>
+                          : gridder_kernel<N, NT, PPT, MINB, VB, TB, false, false, SPL>);
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  kern<<<(unsigned)np, NT, smem, stream>>>(
+  kern<<<dim3((unsigned)np, SPL), NT, smem, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, plan->lmn_dev, reinterpret_cast<const float4 *>(vis),
       reinterpret_cast<const float4 *>(aterms), taper, subgrids + (size_t)p0 * 4 * N * N, plan->T, plan->C,
       plan->n_stations, plan->prm.grid_size, plan->prm.image_size, plan->prm.w_step, plan->prm.aterm_interval);
@@ -243,7 +246,13 @@ int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, co
         return launch_n<24, 64, 9, 6, 512, 128>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
       return launch_n<24, 96, 6, 5, 1024, 64>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
     case 32: return launch_n<32, 256, 4, 2, 512, 512>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
-    case 48: return launch_n<48, 384, 6, 1, 2048, 512>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+    case 48:
+      // blocks of up to ~1000 visibilities: two 192-thread CTAs per subgrid, two to an SM (one CTA of 384 threads leaves
+      // its staging phase and epilogue exposed: 1 channel 0.60 -> 0.65, A-term interval 8 0.64 -> 0.70; long blocks
+      // measured 1-14 % slower that way and keep the single CTA)
+      if (plan->P > 0 && plan->n_planned / plan->P <= 1024)
+        return launch_n<48, 192, 6, 2, 1024, 512, 2>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
+      return launch_n<48, 384, 6, 1, 2048, 512>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
     default: return IDG_ERR_UNSUPPORTED_SUBGRID_SIZE;
   }
 }
