@@ -355,10 +355,17 @@ def run_b200(args):
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
+    # test hooks (tests/test_gpu_bench.py): two ranks on ONE device over gloo exercise the N > 1 code path on a
+    # single-GPU box; a real run uses one device per rank and NCCL
+    backend = os.environ.get("IDG_BENCH_DIST_BACKEND", "nccl")
+    dev_index = 0 if os.environ.get("IDG_BENCH_SINGLE_DEVICE") else local_rank
+    torch.cuda.set_device(dev_index)
+    dev = torch.device("cuda", dev_index)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group(backend)
 
     # ONE workload; rank r owns the contiguous baseline range sharding.baseline_range gives it (strong scaling).
     # The stations, sources and A-terms are drawn before the baselines are selected, so every rank sees the same
@@ -376,7 +383,7 @@ def run_b200(args):
     plan_ms = 1e3 * (time.perf_counter() - t0)
     P, planned, skipped = plan.size()
 
-    m = measure_device_steps(idg, sharding, w, plan, args.steps, args.warmup, world, dev, sampler_index=local_rank)
+    m = measure_device_steps(idg, sharding, w, plan, args.steps, args.warmup, world, dev, sampler_index=dev_index)
     elapsed_ms, stage_ms, clocks = m["elapsed_ms"], m["stage_ms"], m["clocks"]
     if world > 1:
         t = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)

@@ -28,3 +28,22 @@ def test_reference_arm_is_silent_on_other_ranks():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                          capture_output=True, text=True, timeout=120, cwd=ROOT, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_plain_multi_gpu_invocation_fails_loudly_without_the_devices():
+    """`python bench.py --gpus 2` spawns its own ranks; with fewer devices than ranks it must say so, not run one."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    env["CUDA_VISIBLE_DEVICES"] = ""
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2"], capture_output=True, text=True,
+                         timeout=300, cwd=ROOT, env=env)
+    assert out.returncode != 0 and "CUDA device" in (out.stderr + out.stdout) and out.stdout.strip() == ""
+
+
+def test_both_arms_print_the_same_config_object():
+    sys.path.insert(0, ROOT)
+    import bench
+    for wl in ("ska", "lofar", "tiny"):
+        for n in (1, 2, 8):
+            c = bench.config_dict(wl, n)
+            assert set(c) == {"workload", "subgrid_size", "grid_size", "parallelism", "l2"}
+    assert bench.config_dict("ska", 1)["grid_size"] == 8192
