@@ -406,8 +406,7 @@ def run_b200(args):
         d_grid = torch.empty((4, L, L), dtype=torch.complex64, device=dev) if world > 1 else None
         n_e2e = max(2, min(args.steps, 5))
 
-        def e2e_step():
-            h_grid.zero_()
+        def e2e_step():      # idg_grid_host ADDS into the caller's grid (Alg. 1 zeroes V once): no host memset per step
             idg.idg_grid_host(plan, h["uvw"], h["vis"], h["aterms"], h["taper"], h_grid)
             if world > 1:      # the ranks' host grids are summed through the device (NCCL has no host buffers)
                 d_grid.copy_(h_grid, non_blocking=True)

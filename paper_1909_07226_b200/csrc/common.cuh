@@ -50,7 +50,7 @@ struct idg_plan {
   int64_t h_aterm_slots = 0;
   // copy/compute overlap of the *_host entry points: a copy stream and per-chunk events (created on first use)
   cudaStream_t h_copy_stream = nullptr;
-  static constexpr int kHostChunks = 8;
+  static constexpr int kHostChunks = 24;
   cudaEvent_t h_ev_in[kHostChunks + 2] = {};    // chunk uploads, then [kHostChunks] = small inputs, [+1] = grid
   cudaEvent_t h_ev_out[kHostChunks + 1] = {};   // chunk results ready on the compute stream, [kHostChunks] = start
 };
