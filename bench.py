@@ -46,8 +46,9 @@ HBM_FALLBACK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback w
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of the
 # same workload (profiles/r02_ncu_summary.md); None where no capture of that workload exists.
 NCU_TRAFFIC_BYTES = {
-    "ska": {"gridder": None, "degridder": None, "subgrid_fft": None, "adder": None, "splitter_ifft": None},
-    "lofar": {"gridder": 159668480 + 108218624},
+    "ska": {"gridder": int((12.495098 + 8.668407) * 1e9), "degridder": int((16.854431 + 4.237628) * 1e9),
+            "subgrid_fft": None,      # ncu returned no DRAM counters for this launch (two captures); time and bytes only
+            "adder": int((8.862308 + 0.119361) * 1e9), "splitter_ifft": int((0.341461 + 8.651790) * 1e9)},
 }
 
 WORKLOAD_NAMES = {
