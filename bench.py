@@ -162,7 +162,7 @@ def _sample_workload(workload: str):
     parameters) with every k-th baseline only, so that short and long baselines are both in it and nothing of the
     size of the full visibility set is ever built on the host."""
     from paper_1909_07226_b200 import synth
-    stride = {"ska": 64, "paper": 16, "lofar": 4, "sweep": 16}.get(workload, 1)
+    stride = {"ska": 32, "paper": 16, "lofar": 4, "sweep": 16}.get(workload, 1)
     return synth.make_workload(workload, device="cpu", baseline_stride=stride), stride
 
 
