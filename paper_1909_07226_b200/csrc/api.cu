@@ -92,13 +92,14 @@ static int build_adder_lists(idg_plan *pl, cudaStream_t stream) {
 static int finish_plan(idg_plan *pl, const double *freqs_host, cudaStream_t stream) {
   const int N = pl->prm.subgrid_size;
   pl->P = (int64_t)pl->meta_host.size();
-  pl->max_n_time = 0; pl->max_n_chan = 0; pl->n_slots_needed = 0;
+  pl->max_n_time = 0; pl->max_n_chan = 0; pl->min_n_chan = pl->meta_host.empty() ? 0 : INT32_MAX; pl->n_slots_needed = 0;
   pl->sorted_by_baseline = true;
   const bool span = (pl->prm.flags & IDG_PLAN_SPAN_ATERMS) != 0;
   int32_t prev_b = 0;
   for (const auto &m : pl->meta_host) {
     pl->max_n_time = std::max(pl->max_n_time, m.n_time);
     pl->max_n_chan = std::max(pl->max_n_chan, m.n_chan);
+    pl->min_n_chan = std::min(pl->min_n_chan, m.n_chan);
     const int32_t last = span ? (m.time_begin + m.n_time - 1) / pl->prm.aterm_interval : m.aterm_slot;
     pl->n_slots_needed = std::max(pl->n_slots_needed, last + 1);
     if (m.baseline < prev_b) pl->sorted_by_baseline = false;

@@ -28,7 +28,7 @@ struct idg_plan {
   idg_plan_params prm{};
   int32_t B = 0, T = 0, C = 0, n_stations = 0;
   int64_t P = 0, n_planned = 0, n_skipped = 0;
-  int32_t max_n_time = 0, max_n_chan = 0;
+  int32_t max_n_time = 0, max_n_chan = 0, min_n_chan = 0;
   int32_t n_slots_needed = 0;         // A-term slots the metadata indexes (last slot + 1)
   bool planner_made = false;          // metadata from run_planner: sorted by baseline, every sample covered once or skipped
   bool sorted_by_baseline = false;    // baselines non-decreasing in metadata order (the *_host calls chunk by baseline)
@@ -97,6 +97,10 @@ int run_planner(const idg_plan_params &prm, const float *uvw_dev, const double *
 // full [P][4][N][N] array.  The host-buffer entry points use ranges to overlap copies with compute.
 int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
                    const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0 = 0, int64_t np = -1);
+// tensor-core gridder (gridder_tc.cu): N = 32, per-block A-terms, >= 8 channels per block
+bool gridder_tc_eligible(const idg_plan *plan);
+int launch_gridder_tc(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
+                      const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np);
 int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgrids,
                      const float2 *aterms, const float *taper, float2 *vis_out,
                      cudaStream_t stream, int64_t p0 = 0, int64_t np = -1);

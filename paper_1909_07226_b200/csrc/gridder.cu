@@ -237,6 +237,9 @@ int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, co
                    const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
   if (np < 0) np = plan->P - p0;
   if (np <= 0) return IDG_OK;
+  // N = 32, per-block A-terms, at least 8 channels per block: the contraction runs on the tensor cores (gridder_tc.cu;
+  // measured 3-8 % faster than the FFMA2 kernel below on the SKA-like / LOFAR-like plans, same parity)
+  if (gridder_tc_eligible(plan)) return launch_gridder_tc(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
   switch (plan->prm.subgrid_size) {
     case 16: return launch_n<16, 64, 4, 8, 512, 128>(plan, uvw, vis, aterms, taper, subgrids, stream, p0, np);
     case 24:

@@ -662,3 +662,39 @@ def test_error_paths_with_a_device(tiny_case):
     with pytest.raises(idg.IdgError):
         idg.idg_subgrid_fft(c["plan"], c["plan"].subgrids(), 0)           # direction must be -1 or +1
     assert torch.all(g == 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# tensor-core gridder (csrc/gridder_tc.cu): N = 32, >= 8 channels per block
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("uneven,spread", [(False, False), (True, False), (False, True)])
+def test_tensor_core_gridder_ragged_blocks(uneven, spread):
+    """Blocks of 8 / 12 / 16 channels (12 is padded to 16 inside the kernel) and odd timestep counts through the
+    tcgen05 gridder: equally spaced channels take the rotation recurrence, unevenly spaced ones sin/cos per channel;
+    `spread` gives the visibilities of a block twelve orders of magnitude of dynamic range (the kernel scales every
+    block by a power of two into the fp16 range and splits hi + lo)."""
+    w = synth.make_workload("lofar", n_baselines=24, baseline_offset=300, n_time=96)
+    rng = np.random.default_rng(5)
+    if uneven:
+        w.freqs = w.freqs + rng.uniform(-40e3, 40e3, len(w.freqs))
+    if spread:
+        v = w.vis.numpy().copy()
+        v *= (10.0 ** rng.uniform(-6, 6, v.shape[:3]))[..., None].astype(np.float32)
+        w = dataclasses.replace(w, vis=torch.from_numpy(v))
+    d = _np(w)
+    meta, _, _ = orc.plan(w.params, d["uvw"], d["freqs"], w.baselines)
+    meta = meta.copy()
+    meta["n_chan"] = rng.choice([8, 12, 16], len(meta))
+    meta["chan_begin"] = 0
+    meta["n_time"] = np.minimum(meta["n_time"], rng.choice([1, 7, 13, 33, 64], len(meta)))
+    plan = idg.idg_plan_from_metadata(w.params, meta, w.freqs, w.B, w.T, w.n_stations)
+    wc = _cuda(w)
+    ref = orc.gridder(w.params, meta, d["uvw"], d["freqs"], d["vis"], d["aterms"], d["taper"])
+    sub = torch.zeros(ref.shape, dtype=torch.complex64, device="cuda")
+    idg.idg_gridder(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, sub)
+    torch.cuda.synchronize()
+    got = sub.cpu().numpy()
+    err = np.array([H.rel_l2(got[p], ref[p]) for p in range(len(meta))])
+    print("tensor-core gridder worst / median rel-L2: %.2e / %.2e" % (err.max(), np.median(err)))
+    assert err.max() < TOL, (int(err.argmax()), float(err.max()))
