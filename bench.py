@@ -469,6 +469,7 @@ def run_b200(args):
     grid_bytes = 8.0 * 4 * L * L
     extra = {
         "correlations_per_s": 4.0 * value * 1e6,      # 4 polarisations per visibility (BASELINE.json's "0.5 G" reading)
+        "gridder_on_tensor_cores": plan.uses_tensor_cores(),
         "plan_ms": plan_ms, "n_subgrids_rank0": P, "n_vis_rank0": planned, "n_vis_total": total_vis, "n_skipped_rank0": skipped,
         "stage_ms": stage_ms,
         "grid_mvis_s": planned / ((stage_ms["gridder"] + stage_ms["subgrid_fft"] + stage_ms["adder"]) * 1e-3) / 1e6,

@@ -127,6 +127,9 @@ int idg_plan_subgrids(const idg_plan *plan, void **subgrids_dev);
 /* Number of A-term slots the plan indexes: max over subgrids of the last slot + 1 (with IDG_PLAN_SPAN_ATERMS the
  * slot of a block's last timestep decides); 0 for an empty plan. */
 int idg_plan_aterm_slots(const idg_plan *plan, int32_t *n_slots);
+/* 1 if idg_gridder / idg_grid run this plan's contraction on the tensor cores (csrc/gridder_tc.cu: N = 32, one c_p
+ * per block, at least 8 channels in every block, mean block of 256 visibilities or more), 0 if on the FP32 path. */
+int idg_plan_uses_tensor_cores(const idg_plan *plan, int32_t *flag);
 /* w offset of a w layer, w0 = (w_index + 0.5) w_step, or 0 when w_step = 0 (Alg. 1, R4). */
 int idg_plan_w_offset(const idg_plan *plan, int32_t w_index, double *w0);
 void idg_plan_destroy(idg_plan *plan);

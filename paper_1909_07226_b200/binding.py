@@ -23,7 +23,7 @@ assert META_DTYPE.itemsize == 48
 
 EXPORTS = (
     "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_bench_instruction_mix", "idg_plan_create", "idg_plan_from_metadata",
-    "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_aterm_slots", "idg_plan_w_offset",
+    "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_aterm_slots", "idg_plan_w_offset", "idg_plan_uses_tensor_cores",
     "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
     "idg_adder", "idg_splitter", "idg_splitter_ifft", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
@@ -134,6 +134,12 @@ class Plan:
         n = ctypes.c_int32()
         _check(lib().idg_plan_aterm_slots(self.handle, ctypes.byref(n)), "idg_plan_aterm_slots")
         return int(n.value)
+
+    def uses_tensor_cores(self) -> bool:
+        """True if the gridder runs this plan on the tcgen05 path (idg_plan_uses_tensor_cores)."""
+        f = ctypes.c_int32()
+        _check(lib().idg_plan_uses_tensor_cores(self.handle, ctypes.byref(f)), "idg_plan_uses_tensor_cores")
+        return bool(f.value)
 
     def w_offset(self, w_index: int) -> float:
         """w0 of a w layer (idg_plan_w_offset; Alg. 1, R4)."""

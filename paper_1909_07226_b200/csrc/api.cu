@@ -288,6 +288,12 @@ int idg_plan_aterm_slots(const idg_plan *pl, int32_t *n_slots) {
   return IDG_OK;
 }
 
+int idg_plan_uses_tensor_cores(const idg_plan *pl, int32_t *flag) {
+  if (!pl || !flag) return IDG_ERR_INVALID_ARG;
+  *flag = gridder_tc_eligible(pl) ? 1 : 0;
+  return IDG_OK;
+}
+
 int idg_plan_w_offset(const idg_plan *pl, int32_t w_index, double *w0) {
   if (!pl || !w0) return IDG_ERR_INVALID_ARG;
   *w0 = pl->prm.w_step > 0.0 ? ((double)w_index + 0.5) * pl->prm.w_step : 0.0;   // R4

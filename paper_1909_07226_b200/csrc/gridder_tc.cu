@@ -339,7 +339,10 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
 // The tensor-core gridder serves per-block A-terms at N = 32 when every block has at least 8 channels (so that a
 // staging batch holds many more ring slots than the ring is deep); everything else takes gridder_kernel.
 bool gridder_tc_eligible(const idg_plan *plan) {
-  return plan->prm.subgrid_size == 32 && !(plan->prm.flags & IDG_PLAN_SPAN_ATERMS) && plan->min_n_chan >= 8;
+  // blocks shorter than ~256 visibilities do not amortise the pipeline fill and drain of a CTA (sweep: 128-visibility
+  // blocks 0.64 here against 0.71 for the FFMA2 kernel; 256: 0.74 / 0.73; 512: 0.77 / 0.75; 2048: 0.83 / 0.75)
+  return plan->prm.subgrid_size == 32 && !(plan->prm.flags & IDG_PLAN_SPAN_ATERMS) && plan->min_n_chan >= 8 &&
+         plan->P > 0 && plan->n_planned / plan->P >= 256;
 }
 
 int launch_gridder_tc(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,

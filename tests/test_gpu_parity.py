@@ -687,8 +687,9 @@ def test_tensor_core_gridder_ragged_blocks(uneven, spread):
     meta = meta.copy()
     meta["n_chan"] = rng.choice([8, 12, 16], len(meta))
     meta["chan_begin"] = 0
-    meta["n_time"] = np.minimum(meta["n_time"], rng.choice([1, 7, 13, 33, 64], len(meta)))
+    meta["n_time"] = np.minimum(meta["n_time"], rng.choice([13, 21, 33, 64, 64], len(meta)))
     plan = idg.idg_plan_from_metadata(w.params, meta, w.freqs, w.B, w.T, w.n_stations)
+    assert plan.uses_tensor_cores()
     wc = _cuda(w)
     ref = orc.gridder(w.params, meta, d["uvw"], d["freqs"], d["vis"], d["aterms"], d["taper"])
     sub = torch.zeros(ref.shape, dtype=torch.complex64, device="cuda")
