@@ -46,9 +46,9 @@ HBM_FALLBACK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback w
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of the
 # same workload (profiles/r02_ncu_summary.md); None where no capture of that workload exists.
 NCU_TRAFFIC_BYTES = {
-    "ska": {"gridder": int((12.495098 + 8.668407) * 1e9), "degridder": int((16.854431 + 4.237628) * 1e9),
+    "ska": {"gridder": int((15.815207 + 8.678906) * 1e9), "degridder": int((16.854035 + 4.237204) * 1e9),
             "subgrid_fft": None,      # ncu returned no DRAM counters for this launch (two captures); time and bytes only
-            "adder": int((8.862308 + 0.119361) * 1e9), "splitter_ifft": int((0.341461 + 8.651790) * 1e9)},
+            "adder": int((8.862905 + 0.119244) * 1e9), "splitter_ifft": int((0.347184 + 8.652253) * 1e9)},
 }
 
 WORKLOAD_NAMES = {
@@ -309,7 +309,7 @@ def measure_device_steps(idg, sharding, w, plan, steps, warmup, world, dev, samp
             "clocks": clocks}
 
 
-def kernel_rooflines(workload, stage_ms, alone_ms, planned, P, N, touched_px, hbm, hbm_source):
+def kernel_rooflines(workload, stage_ms, alone_ms, planned, P, N, touched_px, hbm, hbm_source, tensor=False):
     """Per-kernel roofline objects: achieved = ALGORITHMIC work per launch / mean launch time inside the timed
     region (36 N^2 flop-equivalents per visibility for gridder / degridder; 64 N^2 bytes per
     subgrid for the FFT; 32 N^2 bytes per subgrid + 64 (32) bytes per touched grid pixel for adder (splitter))."""
@@ -331,7 +331,8 @@ def kernel_rooflines(workload, stage_ms, alone_ms, planned, P, N, touched_px, hb
                     "frac": ach / hbm, "ms": ms, "algorithmic_bytes": nbytes, "traffic": traffic.get(stage),
                     "peak_source": hbm_source})
 
-    alu("gridder_kernel", "gridder")
+    alu("gridder_tc_kernel (tcgen05 contraction; fraction of the FP32 lane-op roofline of the direct evaluation)" if tensor
+        else "gridder_kernel", "gridder")
     alu("degridder_kernel", "degridder")
     mem("subgrid_fft_kernel<N,fwd>", "subgrid_fft", 2 * sub_bytes, stage_ms["subgrid_fft"])
     mem("adder_kernel", "adder", sub_bytes + 2 * px, stage_ms["adder"])
@@ -450,9 +451,10 @@ def run_b200(args):
     hbm_source = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback of B200_PROFILING.md"
     meta = plan.metadata()
     touched_px = touched_grid_pixels(meta, N, L)
-    kernels, alone = kernel_rooflines(args.workload, stage_ms, m["alone_ms"], planned, P, N, touched_px, hbm, hbm_source)
+    tensor = plan.uses_tensor_cores()
+    kernels, alone = kernel_rooflines(args.workload, stage_ms, m["alone_ms"], planned, P, N, touched_px, hbm, hbm_source, tensor)
     g = kernels[0]
-    roofline = {"bound": "alu", "kernel": "gridder_kernel", "achieved": g["achieved"], "peak": ALU_PEAK_TFLOPS,
+    roofline = {"bound": "alu", "kernel": "gridder_tc_kernel" if tensor else "gridder_kernel", "achieved": g["achieved"], "peak": ALU_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": g["frac"], "traffic": g["traffic"], "peak_source": ALU_PEAK_SOURCE,
                 "work": "18 FP32 lane-ops (17 FMA + 1 FMUL) per (visibility, pixel), 2 FLOP-equivalents each",
                 "kernels": kernels}
@@ -462,7 +464,7 @@ def run_b200(args):
         mix = [idg.idg_bench_instruction_mix(4096, v) for v in (0, 1, 2)]
         roofline["measured_mix_peak"] = {
             "tflops": mix[0], "frac_of_alu_peak": mix[0] / ALU_PEAK_TFLOPS, "gridder_frac_of_mix_peak": g["achieved"] / mix[0],
-            "what": "1 FFMA + sin/cos.approx + 8 FFMA2 per (visibility, pixel), operands as in the gridder, no global memory",
+            "what": "1 FFMA + sin/cos.approx + 8 FFMA2 per (visibility, pixel), operands as in the FP32 gridder / degridder, no global memory",
             "uniform_register_operands_tflops": mix[1], "scalar_ffma_tflops": mix[2]}
     except Exception as exc:      # reporting only
         roofline["measured_mix_peak"] = {"error": str(exc)}
@@ -493,7 +495,7 @@ def run_b200(args):
         m2 = measure_device_steps(idg, sharding, w2, p2, max(5, args.steps), args.warmup, 1, dev)
         N2, L2 = w2.params.subgrid_size, w2.params.grid_size
         k2, _ = kernel_rooflines("lofar", m2["stage_ms"], m2["alone_ms"], planned2, P2, N2,
-                                 touched_grid_pixels(p2.metadata(), N2, L2), hbm, hbm_source)
+                                 touched_grid_pixels(p2.metadata(), N2, L2), hbm, hbm_source, p2.uses_tensor_cores())
         ms2 = m2["elapsed_ms"] / max(5, args.steps)
         extra["configs1_lofar"] = {"workload": WORKLOAD_NAMES["lofar"], "value": 2.0 * planned2 / (ms2 * 1e-3) / 1e6,
                                    "unit": UNIT, "ms_per_step": ms2, "stage_ms": m2["stage_ms"], "kernels": k2,
