@@ -14,16 +14,19 @@
 // so one M128 x N16 x K16 MMA covers 128 pixels x 4 visibilities, and the result is D[:, j] + D[:, 8 + j].  The
 // visibilities of a block are scaled by a power of two so that their largest component sits near 2^14 (fp16 range).
 //
-// Structure of a CTA (one subgrid, 288 threads): warps 0-7 generate -- thread (warpgroup g, lane L) owns the pixels
-// (4 g + k) 128 + L, k = 0..3, i.e. row L of four of the eight 128-pixel tiles; per batch of 4 visibilities it
-// evaluates 16 phases (FP64/FP32 split of gridder.cu), sin/cos.approx, splits, and writes its rows of the A tiles
-// straight from registers into a ring slot of tensor memory (tcgen05.st), then arrives on the slot's mbarrier.
-// Warp 8 issues: it waits for the slot, issues the 8 MMAs of the batch (one per pixel tile, all reading the batch's
-// B tile) and commits them to the slot's "empty" mbarrier.  The accumulators D[8 tiles][128 x 16] stay in tensor
-// memory for the whole block; the epilogue reads them back (tcgen05.ld), applies taper and A-terms and stores.
-// The issue rate of a TMEM-operand MMA is ~45 cycles whatever N <= 64 (measured), so the tensor pipe costs 360
-// cycles per batch against ~500 for the 32 MUFU per thread that generate it: the kernel is bound by phasor
-// generation, not by the contraction.
+// Structure of a CTA (HALF a subgrid: 4 pixel tiles of 128, blockIdx.y picks the half; 288 threads, 2 CTAs per SM,
+// 256 tensor-memory columns each: 64 of accumulators + a ring of 3 slots x 64): warps 0-7 generate -- thread
+// (warpgroup g, lane L) owns the pixels (2 g + k) 128 + L, k = 0, 1, i.e. row L of two of the four tiles; per ring slot
+// of 8 visibilities (8 channels of one timestep) it evaluates the phase of the first channel (FP64/FP32 split of
+// gridder.cu) and sin/cos.approx, obtains the other seven phasors by one complex rotation each when the channels are
+// equally spaced (ROT), splits every phasor into fp16 hi + lo, and writes its rows of the A tiles straight from
+// registers into the slot (tcgen05.st), then arrives on the slot's "full" mbarrier.  Warp 8 issues: it waits for the
+// slot, issues the 8 MMAs of the slot (2 batches of 4 visibilities x 4 pixel tiles, each batch reading its 512-byte B
+// tile from shared memory) and commits them to the slot's "empty" mbarrier.  The accumulators D[4 tiles][128 x 16]
+// stay in tensor memory for the whole block; the epilogue reads them back (tcgen05.ld), applies taper and A-terms and
+// stores.  A TMEM-operand MMA costs ~45 cycles whatever N <= 64 (measured: the delivery of the 4 KB A tile), i.e.
+// 0.088 SM-cycles per (visibility, pixel) against 0.19 for the FFMA2 kernel; phasor generation is ~10 instructions
+// per pair.  Measurements and variants: profiles/r02_experiments.md section 7.
 #include <cuda_fp16.h>
 
 #include "common.cuh"
