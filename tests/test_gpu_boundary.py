@@ -259,3 +259,24 @@ def test_guard_bands_planner_made_plan_with_skips():
     for r in meta:
         covered[r["baseline"], r["time_begin"]:r["time_begin"] + r["n_time"], r["chan_begin"]:r["chan_begin"] + r["n_chan"]] = True
     assert np.all(out.cpu().numpy()[~covered] == 0)
+
+
+def test_host_entry_points_with_the_tensor_core_gridder_in_chunks():
+    """A planner-made N = 32 plan that takes the tensor-core gridder, through the chunked host-buffer calls (24
+    baseline ranges, each a launch on a sub-range of the subgrids) against the one-launch device calls."""
+    w = synth.make_workload("lofar", n_baselines=96, baseline_offset=200, n_time=128)
+    wc = w.to("cuda")
+    plan = idg.idg_plan_create(w.params, wc.uvw, w.freqs, w.baselines, w.n_stations)
+    assert plan.uses_tensor_cores()
+    L = w.params.grid_size
+    g_dev = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
+    idg.idg_grid(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, g_dev)
+    g_host = np.zeros((4, L, L), dtype=np.complex64)
+    idg.idg_grid_host(plan, w.uvw.numpy(), w.vis.numpy(), w.aterms.numpy(), w.taper.numpy(), g_host)
+    assert H.rel_l2(g_host, g_dev.cpu().numpy()) < 1e-6
+    v_dev = torch.zeros_like(wc.vis)
+    idg.idg_degrid(plan, wc.uvw, g_dev, wc.aterms, wc.taper, v_dev)
+    v_host = np.zeros(tuple(w.vis.shape), dtype=np.complex64)
+    idg.idg_degrid_host(plan, w.uvw.numpy(), g_dev.cpu().numpy(), w.aterms.numpy(), w.taper.numpy(), v_host)
+    torch.cuda.synchronize()
+    assert np.array_equal(v_host, v_dev.cpu().numpy())
