@@ -4,6 +4,7 @@ device of the box and talk over gloo (NCCL wants one device per rank; the kernel
 one another)."""
 import json
 import os
+import socket
 import subprocess
 import sys
 
@@ -37,10 +38,18 @@ def test_one_rank_line_has_the_contract_keys():
     assert d["detail"]["collective"] is None
 
 
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
 def test_two_ranks_shard_one_workload_and_reduce_the_grid():
     env = dict(os.environ, IDG_BENCH_DIST_BACKEND="gloo", IDG_BENCH_SINGLE_DEVICE="1")
     out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
-                          "--master-addr", "127.0.0.1", "--master-port", "29731", os.path.join(ROOT, "bench.py"),
+                          "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.join(ROOT, "bench.py"),
                           "--gpus", "2", "--workload", "tiny", "--steps", "3", "--warmup", "3"],
                          capture_output=True, text=True, timeout=900, cwd=ROOT, env=env)
     d = _line(out)
