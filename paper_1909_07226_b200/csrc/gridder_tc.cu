@@ -195,8 +195,10 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
           // rows n = p (re), 4 + p (im), 8 + p (re, lo), 12 + p (im, lo); K order cos_hi, sin_hi, cos_lo, sin_lo
           const __half2 re_a = __halves2half2(rh, nih), im_a = __halves2half2(ih, rh);
           const __half2 rel = __halves2half2(rl, nil), iml = __halves2half2(il, rl), zz = __halves2half2(z, z);
-          *reinterpret_cast<uint2 *>(tile + (p) * 16) = make_uint2(*reinterpret_cast<const uint32_t *>(&re_a), *reinterpret_cast<const uint32_t *>(&re_a));
-          *reinterpret_cast<uint2 *>(tile + (4 + p) * 16) = make_uint2(*reinterpret_cast<const uint32_t *>(&im_a), *reinterpret_cast<const uint32_t *>(&im_a));
+          // the cos_lo / sin_lo rows of A hold hi - x = -lo: their B coefficients are negated
+          const __half2 re_n = __hneg2(re_a), im_n = __hneg2(im_a);
+          *reinterpret_cast<uint2 *>(tile + (p) * 16) = make_uint2(*reinterpret_cast<const uint32_t *>(&re_a), *reinterpret_cast<const uint32_t *>(&re_n));
+          *reinterpret_cast<uint2 *>(tile + (4 + p) * 16) = make_uint2(*reinterpret_cast<const uint32_t *>(&im_a), *reinterpret_cast<const uint32_t *>(&im_n));
           *reinterpret_cast<uint2 *>(tile + 256 + (p) * 16) = make_uint2(*reinterpret_cast<const uint32_t *>(&rel), *reinterpret_cast<const uint32_t *>(&zz));
           *reinterpret_cast<uint2 *>(tile + 256 + (4 + p) * 16) = make_uint2(*reinterpret_cast<const uint32_t *>(&iml), *reinterpret_cast<const uint32_t *>(&zz));
         }
@@ -238,9 +240,12 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
                 co[k] = c2;
               }
               const __half2 h = __floats2half2_rn(co[k], si[k]);          // low half = cos (even K), high = sin
-              const float2 hf = __half22float2(h);
-              const __half2 l = __floats2half2_rn(co[k] - hf.x, si[k] - hf.y);
-              areg[k][2 * j] = *reinterpret_cast<const uint32_t *>(&h);
+              const uint32_t hb = *reinterpret_cast<const uint32_t *>(&h);
+              float dc, ds;                                               // hi - x in one mixed-precision add each (FHADD)
+              asm("{ .reg .f16 lo, hi; mov.b32 {lo, hi}, %2; sub.rn.f32.f16 %0, lo, %3; sub.rn.f32.f16 %1, hi, %4; }"
+                  : "=f"(dc), "=f"(ds) : "r"(hb), "f"(co[k]), "f"(si[k]));
+              const __half2 l = __floats2half2_rn(dc, ds);                // = -(x - hi): the sign sits in the B tile
+              areg[k][2 * j] = hb;
               areg[k][2 * j + 1] = *reinterpret_cast<const uint32_t *>(&l);
             }
           }
