@@ -127,6 +127,14 @@ __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
   return *reinterpret_cast<float2 *>(&rd);
 }
 
+__device__ __forceinline__ float2 fmul2(float2 a, float2 b) {
+  unsigned long long ra, rb, rd;
+  ra = *reinterpret_cast<unsigned long long *>(&a);
+  rb = *reinterpret_cast<unsigned long long *>(&b);
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+  return *reinterpret_cast<float2 *>(&rd);
+}
+
 // acc += v * (c + i s) for a complex accumulator, as two FFMA2
 __device__ __forceinline__ void cmac(float2 &acc, float2 v, float c, float s) {
   acc = ffma2(make_float2(v.x, v.x), make_float2(c, s), acc);

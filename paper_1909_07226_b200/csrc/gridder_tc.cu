@@ -230,15 +230,17 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
 #pragma unroll
           for (int j = 0; j < 4 * KB; ++j) {
             const float kd = s_kd[cs * (4 * KB) + j];
+            if (ROT && j > 0) {                                           // (co, si) *= (cr + i sr), both pixels packed
+              static_assert(PPT == 2, "packed rotation over the thread's two pixels");
+              const float2 C = make_float2(co[0], co[1]), S = make_float2(si[0], si[1]);
+              const float2 CR = make_float2(cr[0], cr[1]), SR = make_float2(sr[0], sr[1]);
+              const float2 C2 = ffma2(C, CR, fmul2(S, make_float2(-sr[0], -sr[1])));
+              const float2 S2 = ffma2(S, CR, fmul2(C, SR));
+              co[0] = C2.x; co[1] = C2.y; si[0] = S2.x; si[1] = S2.y;
+            }
 #pragma unroll
             for (int k = 0; k < PPT; ++k) {
-              if (!ROT || j == 0) {
-                __sincosf(fmaf(pidx[k], kd, base[k]), &si[k], &co[k]);
-              } else {                                                    // (co, si) *= (cr + i sr)
-                const float c2 = fmaf(co[k], cr[k], -si[k] * sr[k]);
-                si[k] = fmaf(si[k], cr[k], co[k] * sr[k]);
-                co[k] = c2;
-              }
+              if (!ROT || j == 0) __sincosf(fmaf(pidx[k], kd, base[k]), &si[k], &co[k]);
               const __half2 h = __floats2half2_rn(co[k], si[k]);          // low half = cos (even K), high = sin
               const uint32_t hb = *reinterpret_cast<const uint32_t *>(&h);
               float dc, ds;                                               // hi - x in one mixed-precision add each (FHADD)
