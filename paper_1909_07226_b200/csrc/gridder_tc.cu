@@ -19,14 +19,20 @@
 // (warpgroup g, lane L) owns the pixels (2 g + k) 128 + L, k = 0, 1, i.e. row L of two of the four tiles; per ring slot
 // of 8 visibilities (8 channels of one timestep) it evaluates the phase of the first channel (FP64/FP32 split of
 // gridder.cu) and sin/cos.approx, obtains the other seven phasors by one complex rotation each when the channels are
-// equally spaced (ROT), splits every phasor into fp16 hi + lo, and writes its rows of the A tiles straight from
-// registers into the slot (tcgen05.st), then arrives on the slot's "full" mbarrier.  Warp 8 issues: it waits for the
-// slot, issues the 8 MMAs of the slot (2 batches of 4 visibilities x 4 pixel tiles, each batch reading its 512-byte B
-// tile from shared memory) and commits them to the slot's "empty" mbarrier.  The accumulators D[4 tiles][128 x 16]
-// stay in tensor memory for the whole block; the epilogue reads them back (tcgen05.ld), applies taper and A-terms and
-// stores.  A TMEM-operand MMA costs ~45 cycles whatever N <= 64 (measured: the delivery of the 4 KB A tile), i.e.
-// 0.088 SM-cycles per (visibility, pixel) against 0.19 for the FFMA2 kernel; phasor generation is ~10 instructions
-// per pair.  Measurements and variants: profiles/r02_experiments.md section 7.
+// equally spaced (ROT; both pixels of the thread in one packed f32x2 multiply + FMA pair), splits every phasor into
+// fp16 hi + lo (hi = cvt.f16x2(x); the residual hi - x with one mixed-precision add per component, sub.f32.f16 = FHADD,
+// its sign folded into the B tile; lo = cvt.f16x2 of that), and writes its rows of the A tiles straight from registers
+// into the slot (tcgen05.st), then arrives on the slot's "full" mbarrier.  The terms of the NEXT slot (per-timestep
+// dot products, rotation and anchor sin/cos) are computed in stages between this slot's rotations and the slot's
+// "empty" barrier is tested at the start of the step, so that no shared-memory, MUFU or mbarrier latency sits between
+// two steps of a warp.  Warp 8 issues: it waits for the slot, issues the 8 MMAs of the slot (2 batches of 4
+// visibilities x 4 pixel tiles, each batch reading its 512-byte B tile from shared memory) and commits them to the
+// slot's "empty" mbarrier.  The accumulators D[4 tiles][128 x 16] stay in tensor memory for the whole block; the
+// epilogue reads them back (tcgen05.ld), applies taper and A-terms and stores.  The M128 x N16 x K16 MMA with A in
+// tensor memory runs at its floor of M N / 256 = 8-9 cycles (measured), a tenth of the tensor pipe: the kernel is
+// bound by the generator warps (8 instructions per (visibility, pixel) + ~70 per slot and warp of hand-over), which
+// with 16 generator warps per SM issue on ~60 % of the cycles.  Measurements and variants: profiles/r02_experiments.md
+// section 7.
 #include <cuda_fp16.h>
 
 #include "common.cuh"
@@ -59,6 +65,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
   for (int spins = 0; spins < (1 << 26); ++spins) {        // bounded: a lost arrival traps instead of hanging the GPU
     asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                  : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    if (ok) return;
+  }
+  __trap();
+}
+__device__ __forceinline__ void mbar_wait_addr(uint32_t addr, uint32_t parity) {
+  uint32_t ok = 0;
+  for (int spins = 0; spins < (1 << 26); ++spins) {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
     if (ok) return;
   }
   __trap();
@@ -171,7 +186,9 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
       const float4 q = __ldg(&lmn[pix_base + (PPT * g + k) * 128 + Lrow]);
       ql[k] = q.x; qm[k] = q.y; qn[k] = q.z;
     }
-    int gs = 0;                                                // ring-slot counter of the block
+    uint32_t slot = 0, round = 0;                              // ring slot of the next step; times the ring went round
+    uint32_t empty_base = smem_u32(&bar_empty[0]), full_base = smem_u32(&bar_full[0]);
+    asm volatile("" : "+r"(empty_base), "+r"(full_base));      // kept in registers (not rematerialised per slot)
     for (int t0 = 0, sb = 0; t0 < n_time; t0 += tb_max, ++sb) {
       const int tb = min(tb_max, n_time - t0), buf = sb & 1;
       unsigned char *bt = s_b + buf * (kSmemB / 2);
@@ -212,24 +229,62 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the MMAs read the B tiles through the async proxy
       asm volatile("bar.sync 1, 256;" ::: "memory");                   // generators only
-      // ---- generate: per timestep, per ring slot of 4 KB channels
-      for (int tl = 0; tl < tb; ++tl) {
+      // ---- generate: per timestep, per ring slot of 4 KB channels.  Software-pipelined: the per-timestep terms and
+      // the anchor sin/cos of the NEXT slot are started before this slot's rotations, and the slot's "empty" barrier
+      // is tested early, so that none of those latencies sits between two slots of a warp.
+      float npidx[PPT], nbase[PPT], ncr[PPT], nsr[PPT], nco[PPT], nsi[PPT];
+      auto prep_time = [&](int tl) {
         const float4 tu = st[2 * tl], tbs = st[2 * tl + 1];
-        float pidx[PPT], base[PPT], cr[PPT], sr[PPT];
 #pragma unroll
         for (int k = 0; k < PPT; ++k) {
-          pidx[k] = fmaf(tu.x, ql[k], fmaf(tu.y, qm[k], tu.z * qn[k]));
-          base[k] = fmaf(tbs.x, ql[k], fmaf(tbs.y, qm[k], tbs.z * qn[k]));
-          if (ROT) __sincosf(pidx[k] * dkd, &sr[k], &cr[k]);
+          npidx[k] = fmaf(tu.x, ql[k], fmaf(tu.y, qm[k], tu.z * qn[k]));
+          nbase[k] = fmaf(tbs.x, ql[k], fmaf(tbs.y, qm[k], tbs.z * qn[k]));
+          if (ROT) __sincosf(npidx[k] * dkd, &nsr[k], &ncr[k]);
         }
-        for (int cs = 0; cs < spt; ++cs, ++gs) {
-          const int slot = gs % RING;
-          if (gs >= RING) { mbar_wait(&bar_empty[slot], ((gs / RING) - 1) & 1); tc_fence_after(); }
+      };
+      auto prep_anchor = [&](int cs) {
+        const float kd = s_kd[cs * (4 * KB)];
+#pragma unroll
+        for (int k = 0; k < PPT; ++k) __sincosf(fmaf(npidx[k], kd, nbase[k]), &nsi[k], &nco[k]);
+      };
+      prep_time(0);
+      prep_anchor(0);
+      for (int tl = 0; tl < tb; ++tl) {
+        for (int cs = 0; cs < spt; ++cs) {
+          float pidx[PPT], base[PPT], cr[PPT], sr[PPT], co[PPT], si[PPT];
+#pragma unroll
+          for (int k = 0; k < PPT; ++k) {
+            pidx[k] = npidx[k]; base[k] = nbase[k]; cr[k] = ncr[k]; sr[k] = nsr[k]; co[k] = nco[k]; si[k] = nsi[k];
+          }
+          const uint32_t empty_addr = empty_base + 8u * slot;
+          uint32_t slot_free = 1;
+          if (round > 0)                                                  // non-blocking; consumed before the stores
+            asm volatile("{ .reg .pred p; mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(slot_free) : "r"(empty_addr), "r"((round - 1) & 1u) : "memory");
+          // next slot: (tl, cs + 1) or (tl + 1, 0); its terms are computed in stages between this slot's rotations
+          const bool new_time = cs + 1 == spt;
+          const int ncs = new_time ? 0 : cs + 1, ntl = min(tl + (new_time ? 1 : 0), tb - 1);
+          float4 tu, tbs;
+          float nkd;
           uint32_t areg[PPT][8 * KB];
-          float co[PPT], si[PPT];
 #pragma unroll
           for (int j = 0; j < 4 * KB; ++j) {
-            const float kd = s_kd[cs * (4 * KB) + j];
+            if (j == 0) { tu = st[2 * ntl]; tbs = st[2 * ntl + 1]; nkd = s_kd[ncs * (4 * KB)]; }
+            if (j == 2 && new_time) {
+#pragma unroll
+              for (int k = 0; k < PPT; ++k) {
+                npidx[k] = fmaf(tu.x, ql[k], fmaf(tu.y, qm[k], tu.z * qn[k]));
+                nbase[k] = fmaf(tbs.x, ql[k], fmaf(tbs.y, qm[k], tbs.z * qn[k]));
+              }
+            }
+            if (j == 3 && new_time && ROT) {
+#pragma unroll
+              for (int k = 0; k < PPT; ++k) __sincosf(npidx[k] * dkd, &nsr[k], &ncr[k]);
+            }
+            if (j == 4) {
+#pragma unroll
+              for (int k = 0; k < PPT; ++k) __sincosf(fmaf(npidx[k], nkd, nbase[k]), &nsi[k], &nco[k]);
+            }
             if (ROT && j > 0) {                                           // (co, si) *= (cr + i sr), both pixels packed
               static_assert(PPT == 2, "packed rotation over the thread's two pixels");
               const float2 C = make_float2(co[0], co[1]), S = make_float2(si[0], si[1]);
@@ -240,7 +295,7 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
             }
 #pragma unroll
             for (int k = 0; k < PPT; ++k) {
-              if (!ROT || j == 0) __sincosf(fmaf(pidx[k], kd, base[k]), &si[k], &co[k]);
+              if (!ROT && j > 0) __sincosf(fmaf(pidx[k], s_kd[cs * (4 * KB) + j], base[k]), &si[k], &co[k]);
               const __half2 h = __floats2half2_rn(co[k], si[k]);          // low half = cos (even K), high = sin
               const uint32_t hb = *reinterpret_cast<const uint32_t *>(&h);
               float dc, ds;                                               // hi - x in one mixed-precision add each (FHADD)
@@ -251,19 +306,23 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
               areg[k][2 * j + 1] = *reinterpret_cast<const uint32_t *>(&l);
             }
           }
+          if (!slot_free) mbar_wait_addr(empty_addr, (round - 1) & 1u);
+          tc_fence_after();
 #pragma unroll
           for (int k = 0; k < PPT; ++k) {
-            const uint32_t ta = tmem + lane_base + (uint32_t)(COLS_D + slot * COLS_SLOT + (PPT * g + k) * (8 * KB));
+            const uint32_t ta = tmem + lane_base + (uint32_t)(COLS_D + (PPT * g + k) * (8 * KB)) + slot * (uint32_t)COLS_SLOT;
             static_assert(KB == 2, "one tcgen05.st.x16 per tile");
             asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
                          ::"r"(ta), "r"(areg[k][0]), "r"(areg[k][1]), "r"(areg[k][2]), "r"(areg[k][3]), "r"(areg[k][4]),
-                         "r"(areg[k][5]), "r"(areg[k][6]), "r"(areg[k][7]), "r"(areg[k][8]), "r"(areg[k][9]), "r"(areg[k][10]),
-                         "r"(areg[k][11]), "r"(areg[k][12]), "r"(areg[k][13]), "r"(areg[k][14]), "r"(areg[k][15]) : "memory");
+                           "r"(areg[k][5]), "r"(areg[k][6]), "r"(areg[k][7]), "r"(areg[k][8]), "r"(areg[k][9]), "r"(areg[k][10]),
+                           "r"(areg[k][11]), "r"(areg[k][12]), "r"(areg[k][13]), "r"(areg[k][14]), "r"(areg[k][15]) : "memory");
           }
           asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(&bar_full[slot]);
+          if (lane == 0)
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_base + 8u * slot) : "memory");
+          if (++slot == RING) { slot = 0; ++round; }
         }
       }
     }
