@@ -14,8 +14,10 @@
 // so one M128 x N16 x K16 MMA covers 128 pixels x 4 visibilities, and the result is D[:, j] + D[:, 8 + j].  The
 // visibilities of a block are scaled by a power of two so that their largest component sits near 2^14 (fp16 range).
 //
-// Structure of a CTA (HALF a subgrid: 4 pixel tiles of 128, blockIdx.y picks the half; 288 threads, 2 CTAs per SM,
-// 256 tensor-memory columns each: 64 of accumulators + a ring of 3 slots x 64): warps 0-7 generate -- thread
+// Structure of a CTA (HALF a subgrid: 4 pixel tiles of 128, blockIdx.y picks the half; 288 threads at 72 registers and
+// 128 tensor-memory columns -- 64 of accumulators + ONE slot of 64 -- so that THREE CTAs share an SM: the generator
+// warps are latency-bound, and 24 of them per SM with a single slot beat 16 with a ring of three by 8 %): warps 0-7
+// generate -- thread
 // (warpgroup g, lane L) owns the pixels (2 g + k) 128 + L, k = 0, 1, i.e. row L of two of the four tiles; per ring slot
 // of 8 visibilities (8 channels of one timestep) it evaluates the phase of the first channel (FP64/FP32 split of
 // gridder.cu) and sin/cos.approx, obtains the other seven phasors by one complex rotation each when the channels are
@@ -30,8 +32,8 @@
 // slot's "empty" mbarrier.  The accumulators D[4 tiles][128 x 16] stay in tensor memory for the whole block; the
 // epilogue reads them back (tcgen05.ld), applies taper and A-terms and stores.  The M128 x N16 x K16 MMA with A in
 // tensor memory runs at its floor of M N / 256 = 8-9 cycles (measured), a tenth of the tensor pipe: the kernel is
-// bound by the generator warps (8 instructions per (visibility, pixel) + ~70 per slot and warp of hand-over), which
-// with 16 generator warps per SM issue on ~60 % of the cycles.  Measurements and variants: profiles/r02_experiments.md
+// bound by the generator warps (6 issue slots per (visibility, pixel) + ~70 per slot and warp of hand-over), which
+// issued on ~60 % of the cycles with 16 generator warps per SM (two CTAs of 256 columns).  Measurements and variants: profiles/r02_experiments.md
 // section 7.
 #include <cuda_fp16.h>
 
@@ -109,12 +111,12 @@ using namespace tc;
 // from one complex rotation by exp(i pidx dkd) each (4 FP32 ops instead of 1 FMA + 1 FMUL + 2 MUFU; seven
 // rotations add ~1e-6 of phase error), which takes the kernel off the MUFU bound.
 template <int RING, bool ROT>
-__global__ void __launch_bounds__(tc::NT, 2)
+__global__ void __launch_bounds__(tc::NT, 3)
 gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                   const double *__restrict__ freqs, const float4 *__restrict__ lmn, const float4 *__restrict__ vis,
                   const float4 *__restrict__ aterms, const float *__restrict__ taper, float2 *__restrict__ subgrids,
                   int32_t T, int32_t C, int32_t n_stations, int32_t L, double image_size, double w_step, float dkd) {
-  constexpr int TMEM_COLS = 256;
+  constexpr int TMEM_COLS = 128;
   static_assert(COLS_D + RING * COLS_SLOT <= TMEM_COLS, "ring does not fit the tensor-memory allocation");
   extern __shared__ __align__(128) unsigned char smem_dyn[];
   unsigned char *s_b = smem_dyn;                                          // [2][VS / 4][512]: B tiles, two staging buffers
@@ -416,7 +418,7 @@ bool gridder_tc_eligible(const idg_plan *plan) {
 
 int launch_gridder_tc(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
                       const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np) {
-  constexpr int RING = 3;
+  constexpr int RING = 1;
   const bool rot = plan->uniform_dkd != 0.f;
   auto kern = rot ? gridder_tc_kernel<RING, true> : gridder_tc_kernel<RING, false>;
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
