@@ -48,7 +48,7 @@ constexpr int SPL = 2;                                      // CTAs per subgrid 
 constexpr int TILES = NPIX / 128 / SPL;                     // 4 pixel tiles of 128 (MMA M) per CTA
 constexpr int GEN_THREADS = 256, NT = GEN_THREADS + 32;     // 8 generator warps + the issuing warp
 constexpr int PPT = TILES * 128 / GEN_THREADS;              // 2 pixels per generator thread
-constexpr int VS = 256;                                     // visibilities per staging batch (64 B tiles of 512 bytes)
+constexpr int VS = 128;                                     // visibilities per staging batch (32 B tiles of 512 bytes)
 constexpr int KB = 2;                                       // MMA batches (of 4 visibilities) per ring slot
 constexpr int COLS_D = TILES * 16;                          // accumulator columns: 64
 constexpr int COLS_SLOT = TILES * 8 * KB;                   // A columns per ring slot: [tile][batch][K16 fp16 = 8 x 32-bit]
@@ -111,7 +111,7 @@ using namespace tc;
 // from one complex rotation by exp(i pidx dkd) each (4 FP32 ops instead of 1 FMA + 1 FMUL + 2 MUFU; seven
 // rotations add ~1e-6 of phase error), which takes the kernel off the MUFU bound.
 template <int RING, bool ROT>
-__global__ void __launch_bounds__(tc::NT, 3)
+__global__ void __launch_bounds__(tc::NT, 4)
 gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__restrict__ uvw,
                   const double *__restrict__ freqs, const float4 *__restrict__ lmn, const float4 *__restrict__ vis,
                   const float4 *__restrict__ aterms, const float *__restrict__ taper, float2 *__restrict__ subgrids,
@@ -307,17 +307,20 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
               areg[k][2 * j] = hb;
               areg[k][2 * j + 1] = *reinterpret_cast<const uint32_t *>(&l);
             }
-          }
-          if (!slot_free) mbar_wait_addr(empty_addr, (round - 1) & 1u);
-          tc_fence_after();
+            if ((j & 3) == 3) {                                           // 4 visibilities done: one MMA batch of rows
+              if (j == 3) {
+                if (!slot_free) mbar_wait_addr(empty_addr, (round - 1) & 1u);
+                tc_fence_after();
+              }
 #pragma unroll
-          for (int k = 0; k < PPT; ++k) {
-            const uint32_t ta = tmem + lane_base + (uint32_t)(COLS_D + (PPT * g + k) * (8 * KB)) + slot * (uint32_t)COLS_SLOT;
-            static_assert(KB == 2, "one tcgen05.st.x16 per tile");
-            asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-                         ::"r"(ta), "r"(areg[k][0]), "r"(areg[k][1]), "r"(areg[k][2]), "r"(areg[k][3]), "r"(areg[k][4]),
-                           "r"(areg[k][5]), "r"(areg[k][6]), "r"(areg[k][7]), "r"(areg[k][8]), "r"(areg[k][9]), "r"(areg[k][10]),
-                           "r"(areg[k][11]), "r"(areg[k][12]), "r"(areg[k][13]), "r"(areg[k][14]), "r"(areg[k][15]) : "memory");
+              for (int k = 0; k < PPT; ++k) {
+                const int r0 = 2 * (j - 3);
+                const uint32_t ta = tmem + lane_base + (uint32_t)(COLS_D + (PPT * g + k) * (8 * KB) + r0) + slot * (uint32_t)COLS_SLOT;
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                             ::"r"(ta), "r"(areg[k][r0]), "r"(areg[k][r0 + 1]), "r"(areg[k][r0 + 2]), "r"(areg[k][r0 + 3]),
+                               "r"(areg[k][r0 + 4]), "r"(areg[k][r0 + 5]), "r"(areg[k][r0 + 6]), "r"(areg[k][r0 + 7]) : "memory");
+              }
+            }
           }
           asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
           tc_fence_before();
@@ -413,6 +416,7 @@ bool gridder_tc_eligible(const idg_plan *plan) {
   // blocks shorter than ~256 visibilities do not amortise the pipeline fill and drain of a CTA (sweep: 128-visibility
   // blocks 0.64 here against 0.71 for the FFMA2 kernel; 256: 0.74 / 0.73; 512: 0.77 / 0.75; 2048: 0.83 / 0.75)
   return plan->prm.subgrid_size == 32 && !(plan->prm.flags & IDG_PLAN_SPAN_ATERMS) && plan->min_n_chan >= 8 &&
+         plan->max_n_chan <= tc::VS &&                  // a staging batch holds at least one timestep of the block
          plan->P > 0 && plan->n_planned / plan->P >= 256;
 }
 
@@ -422,6 +426,7 @@ int launch_gridder_tc(const idg_plan *plan, const float *uvw, const float2 *vis,
   const bool rot = plan->uniform_dkd != 0.f;
   auto kern = rot ? gridder_tc_kernel<RING, true> : gridder_tc_kernel<RING, false>;
   IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
+  IDG_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   kern<<<dim3((unsigned)np, tc::SPL), tc::NT, kSmem, stream>>>(
       plan->meta_dev + p0, uvw, plan->freqs_dev, plan->lmn_dev, reinterpret_cast<const float4 *>(vis),
       reinterpret_cast<const float4 *>(aterms), taper, subgrids + (size_t)p0 * 4 * tc::NPIX, plan->T, plan->C,
