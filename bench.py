@@ -417,27 +417,45 @@ def run_b200(args):
                 torch.cuda.synchronize()
             idg.idg_degrid_host(plan, h["uvw"], h_grid, h["aterms"], h["taper"], h_out)
 
-        e2e_step()                                              # warm-up (allocates the plan's staging buffers)
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            e2e_step()
-        torch.cuda.synchronize()
-        e2e_s = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        def fused_step():    # one imaging cycle with the grid resident on the device; grid and visibilities come back
+            idg.idg_grid_degrid_host(plan, h["uvw"], h["vis"], h["aterms"], h["taper"], h_grid, h_out)
+
+        def time_steps(fn):
+            fn()                                                # warm-up (allocates the plan's staging buffers)
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+            t0 = time.perf_counter()
+            for _ in range(n_e2e):
+                fn()
+            torch.cuda.synchronize()
+            sec = (time.perf_counter() - t0) / n_e2e
+            if world > 1:
+                t = torch.tensor([sec], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                sec = float(t.item())
+            return sec
+
         nb = lambda x: x.numel() * x.element_size()
+        two_s = time_steps(e2e_step)
         h2d = 2 * (nb(h["uvw"]) + nb(h["aterms"]) + nb(h["taper"]) + nb(h_grid)) + nb(h["vis"])
         d2h = nb(h_grid) + nb(h_out)
         if world > 1:
             h2d += nb(h_grid); d2h += nb(h_grid)
-        e2e = {"value": 2.0 * total_vis / e2e_s / 1e6, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_s, "steps": n_e2e,
+        two = {"value": 2.0 * total_vis / two_s / 1e6, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * two_s, "steps": n_e2e,
                "what": "idg_grid_host + idg_degrid_host on pinned host buffers (per rank), copies inside the timed region"}
+        if world == 1:
+            # the grid of one rank is the whole grid: the cycle runs as ONE call that keeps it on the device
+            one_s = time_steps(fused_step)
+            e2e = {"value": 2.0 * total_vis / one_s / 1e6, "unit": UNIT,
+                   "h2d_bytes_per_step": int(nb(h["uvw"]) + nb(h["aterms"]) + nb(h["taper"]) + nb(h["vis"])),
+                   "d2h_bytes_per_step": int(nb(h_grid) + nb(h_out)), "ms_per_step": 1e3 * one_s, "steps": n_e2e,
+                   "what": "idg_grid_degrid_host on pinned host buffers: inputs up once, grid resident on the device, "
+                           "grid and predicted visibilities copied back, copies inside the timed region",
+                   "two_calls": two}
+        else:
+            e2e = two
         del h, h_grid, h_out, d_grid
 
     if rank != 0:

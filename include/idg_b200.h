@@ -155,6 +155,17 @@ int idg_degrid_host(idg_plan *plan, const float *uvw_host, const void *grid_host
                     const void *aterms_host, int32_t n_slots, const float *taper_host,
                     void *vis_out_host, void *cuda_stream);
 
+/* ---- one imaging cycle on HOST buffers with the grid resident on the device: Alg. 1 of
+ * vis_host into a ZEROED device grid, then Alg. 2 from that grid into vis_out_host.
+ *   grid_host     [4][L][L] complex64, host, OPTIONAL (NULL: the grid is not copied back): receives the grid
+ *                 (overwritten, not accumulated into)
+ *   vis_out_host  [B][T][C][4] complex64, host: the predicted visibilities (skipped ones 0); may alias vis_host
+ * Inputs are uploaded once, the copies overlap the kernels in both directions; synchronises like the other
+ * *_host calls; same error behaviour. */
+int idg_grid_degrid_host(idg_plan *plan, const float *uvw_host, const void *vis_host,
+                         const void *aterms_host, int32_t n_slots, const float *taper_host,
+                         void *grid_host, void *vis_out_host, void *cuda_stream);
+
 /* ---- stage-level entry points (parity tests, per-stage timing); same conventions ------------
  * a1 gridder: Eq. 25, Alg. 1, section 3.4 PAPER.md:247-249:
  *   Sg[y][x] = taper A1^H (sum_k Y_k exp(+2 pi i (du l_x + dv m_y + dw n'_xy))) A2  -> subgrids */

@@ -25,7 +25,7 @@ EXPORTS = (
     "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_bench_instruction_mix", "idg_plan_create", "idg_plan_from_metadata",
     "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_aterm_slots", "idg_plan_w_offset", "idg_plan_uses_tensor_cores",
     "idg_plan_destroy", "idg_grid",
-    "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_gridder", "idg_subgrid_fft",
+    "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_grid_degrid_host", "idg_gridder", "idg_subgrid_fft",
     "idg_adder", "idg_splitter", "idg_splitter_ifft", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
     "idg_image_divide", "idg_image_taper", "idg_taper_optimal", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
 
@@ -325,6 +325,25 @@ def idg_degrid_host(plan: Plan, uvw, grid, aterms, taper, vis_out, stream=None) 
         raise IdgError("vis_out must be a contiguous complex64 array (it is written in place)")
     _check(lib().idg_degrid_host(plan.handle, up, gp, ap, ctypes.c_int32(int(aterms.shape[0])), tp, vp,
                                  _stream(stream)), "idg_degrid_host")
+
+
+def idg_grid_degrid_host(plan: Plan, uvw, vis, aterms, taper, grid, vis_out, stream=None) -> None:
+    """Alg. 1 then Alg. 2 on HOST buffers with the grid resident on the device; grid may be None (not copied back),
+    otherwise it is overwritten with the grid of `vis`; vis_out receives the predicted visibilities."""
+    _shape_check(plan, uvw=uvw, vis=vis, aterms=aterms, taper=taper)
+    _shape_check(plan, vis=vis_out)
+    up, k1 = _host(uvw, np.float32, "uvw"); vp, k2 = _host_c64(vis, "vis"); ap, k3 = _host_c64(aterms, "aterms")
+    tp, k4 = _host(taper, np.float32, "taper"); op, k5 = _host_c64(vis_out, "vis_out")
+    if isinstance(vis_out, np.ndarray) and k5 is not vis_out:
+        raise IdgError("vis_out must be a contiguous complex64 array (it is written in place)")
+    gp, k6 = None, None
+    if grid is not None:
+        _shape_check(plan, grid=grid)
+        gp, k6 = _host_c64(grid, "grid")
+        if isinstance(grid, np.ndarray) and k6 is not grid:
+            raise IdgError("grid must be a contiguous complex64 array (it is written in place)")
+    _check(lib().idg_grid_degrid_host(plan.handle, up, vp, ap, ctypes.c_int32(int(aterms.shape[0])), tp, gp, op,
+                                      _stream(stream)), "idg_grid_degrid_host")
 
 
 def idg_image_w_accumulate(acc, layer, image_size: float, w0: float, sign: int = 1, stream=None) -> None:

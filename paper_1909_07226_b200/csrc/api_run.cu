@@ -274,6 +274,74 @@ static int degrid_host_impl(idg_plan *pl, const float *uvw_host, const void *gri
   return IDG_OK;
 }
 
+// Alg. 1 followed by Alg. 2 with the grid RESIDENT on the device: the small inputs and the visibilities go up once
+// (chunk k is gridded while chunk k + 1 travels), the adder runs into a zeroed device grid, the grid travels back on
+// the copy stream (if the caller wants it) while the chunks are predicted from the device copy, and chunk k's
+// visibilities travel back while chunk k + 1 is predicted.  Against idg_grid_host + idg_degrid_host this saves one
+// upload and (with grid_host == NULL) one download of the grid and the second upload of uvw / A-terms / taper.
+static int grid_degrid_host_impl(idg_plan *pl, const float *uvw_host, const void *vis_host, const void *aterms_host,
+                                 int32_t n_slots, const float *taper_host, void *grid_host, void *vis_out_host,
+                                 void *stream) {
+  if (!pl || !uvw_host || !vis_host || !aterms_host || !taper_host || !vis_out_host) return IDG_ERR_INVALID_ARG;
+  if (n_slots < pl->n_slots_needed) return IDG_ERR_PLAN_MISMATCH;
+  int rc = ensure_staging(pl, n_slots);
+  if (rc == IDG_OK) rc = ensure_host_pipeline(pl);
+  if (rc != IDG_OK) return rc;
+  const size_t N = pl->prm.subgrid_size, L = pl->prm.grid_size;
+  const size_t row = (size_t)pl->T * pl->C * 4;
+  const size_t nvis = (size_t)pl->B * pl->T * pl->C;
+  cudaStream_t s = S(stream), c = pl->h_copy_stream;
+  const auto chunks = host_chunks(pl);
+  const int K = idg_plan::kHostChunks;
+  IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_out[K], s));
+  IDG_CUDA_TRY(cudaStreamWaitEvent(c, pl->h_ev_out[K], 0));
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_uvw_dev, uvw_host, sizeof(float) * 3 * (size_t)pl->B * pl->T, cudaMemcpyHostToDevice, c));
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_aterms_dev, aterms_host, sizeof(float2) * 4 * N * N * (size_t)pl->n_stations * n_slots, cudaMemcpyHostToDevice, c));
+  IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_taper_dev, taper_host, sizeof(float) * N * N, cudaMemcpyHostToDevice, c));
+  IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_in[K], c));
+  for (size_t k = 0; k < chunks.size(); ++k) {
+    const HostChunk &ch = chunks[k];
+    IDG_CUDA_TRY(cudaMemcpyAsync(pl->h_vis_dev + (size_t)ch.b0 * row, (const float2 *)vis_host + (size_t)ch.b0 * row,
+                                 sizeof(float2) * row * (size_t)(ch.b1 - ch.b0), cudaMemcpyHostToDevice, c));
+    IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_in[k], c));
+  }
+  // ---- Alg. 1 into a zeroed device grid
+  IDG_CUDA_TRY(cudaMemsetAsync(pl->h_grid_dev, 0, sizeof(float2) * 4 * L * L, s));
+  IDG_CUDA_TRY(cudaStreamWaitEvent(s, pl->h_ev_in[K], 0));
+  for (size_t k = 0; k < chunks.size(); ++k) {
+    const HostChunk &ch = chunks[k];
+    IDG_CUDA_TRY(cudaStreamWaitEvent(s, pl->h_ev_in[k], 0));
+    rc = launch_gridder(pl, pl->h_uvw_dev, pl->h_vis_dev, pl->h_aterms_dev, pl->h_taper_dev, pl->subgrids_dev, s,
+                        ch.p0, ch.p1 - ch.p0);
+    if (rc == IDG_OK) rc = launch_subgrid_fft(pl, pl->subgrids_dev, -1, s, ch.p0, ch.p1 - ch.p0);
+    if (rc != IDG_OK) return rc;
+  }
+  rc = launch_adder(pl, pl->subgrids_dev, pl->h_grid_dev, s);
+  if (rc != IDG_OK) return rc;
+  IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_in[K + 1], s));          // the grid is complete
+  IDG_CUDA_TRY(cudaStreamWaitEvent(c, pl->h_ev_in[K + 1], 0));
+  if (grid_host)
+    IDG_CUDA_TRY(cudaMemcpyAsync(grid_host, pl->h_grid_dev, sizeof(float2) * 4 * L * L, cudaMemcpyDeviceToHost, c));
+  // ---- Alg. 2 from the device grid; the staging buffer of the measured visibilities receives the predicted ones
+  if (pl->n_skipped > 0 || !pl->planner_made)
+    IDG_CUDA_TRY(cudaMemsetAsync(pl->h_vis_dev, 0, sizeof(float2) * 4 * nvis, s));
+  for (size_t k = 0; k < chunks.size(); ++k) {
+    const HostChunk &ch = chunks[k];
+    rc = launch_splitter_ifft(pl, pl->h_grid_dev, pl->subgrids_dev, s, ch.p0, ch.p1 - ch.p0);
+    if (rc == IDG_OK)
+      rc = launch_degridder(pl, pl->h_uvw_dev, pl->subgrids_dev, pl->h_aterms_dev, pl->h_taper_dev, pl->h_vis_dev, s,
+                            ch.p0, ch.p1 - ch.p0);
+    if (rc != IDG_OK) return rc;
+    IDG_CUDA_TRY(cudaEventRecord(pl->h_ev_out[k], s));
+    IDG_CUDA_TRY(cudaStreamWaitEvent(c, pl->h_ev_out[k], 0));
+    IDG_CUDA_TRY(cudaMemcpyAsync((float2 *)vis_out_host + (size_t)ch.b0 * row, pl->h_vis_dev + (size_t)ch.b0 * row,
+                                 sizeof(float2) * row * (size_t)(ch.b1 - ch.b0), cudaMemcpyDeviceToHost, c));
+  }
+  IDG_CUDA_TRY(cudaStreamSynchronize(s));
+  IDG_CUDA_TRY(cudaStreamSynchronize(c));
+  return IDG_OK;
+}
+
 // On failure the asynchronous copies already queued still reference the caller's host buffers: both streams are
 // drained before the error is returned, so the caller may free them.
 static int host_call_epilogue(idg_plan *pl, void *stream, int rc) {
@@ -298,6 +366,15 @@ int idg_degrid_host(idg_plan *pl, const float *uvw_host, const void *grid_host, 
   int rc;
   try {
     rc = degrid_host_impl(pl, uvw_host, grid_host, aterms_host, n_slots, taper_host, vis_out_host, stream);
+  } catch (const std::bad_alloc &) { rc = IDG_ERR_OUT_OF_MEMORY; } catch (...) { rc = IDG_ERR_INVALID_ARG; }
+  return host_call_epilogue(pl, stream, rc);
+}
+
+int idg_grid_degrid_host(idg_plan *pl, const float *uvw_host, const void *vis_host, const void *aterms_host,
+                         int32_t n_slots, const float *taper_host, void *grid_host, void *vis_out_host, void *stream) {
+  int rc;
+  try {
+    rc = grid_degrid_host_impl(pl, uvw_host, vis_host, aterms_host, n_slots, taper_host, grid_host, vis_out_host, stream);
   } catch (const std::bad_alloc &) { rc = IDG_ERR_OUT_OF_MEMORY; } catch (...) { rc = IDG_ERR_INVALID_ARG; }
   return host_call_epilogue(pl, stream, rc);
 }

@@ -360,6 +360,31 @@ def test_host_entry_points_match_device_entry_points(tiny_case):
     assert np.array_equal(v_host, v_dev.cpu().numpy())
 
 
+def test_fused_host_cycle_matches_the_two_calls(tiny_case):
+    """idg_grid_degrid_host (grid resident on the device) = idg_grid_host into a zero grid, then idg_degrid_host of
+    that grid: the same kernels in the same order; the adder's atomics are the only difference (FP32 sums in another
+    order), hence 1e-6 instead of equality.  With grid=None the visibilities are the same and nothing else is written."""
+    c = tiny_case
+    L = c["prm"].grid_size
+    d = c["d"]
+    g_ref = np.zeros((4, L, L), dtype=np.complex64)
+    idg.idg_grid_host(c["plan"], d["uvw"], d["vis"], d["aterms"], d["taper"], g_ref)
+    v_ref = np.zeros(d["vis"].shape, dtype=np.complex64)
+    idg.idg_degrid_host(c["plan"], d["uvw"], g_ref, d["aterms"], d["taper"], v_ref)
+    g = np.full((4, L, L), 7 + 7j, dtype=np.complex64)            # overwritten, not accumulated into
+    v = np.zeros(d["vis"].shape, dtype=np.complex64)
+    idg.idg_grid_degrid_host(c["plan"], d["uvw"], d["vis"], d["aterms"], d["taper"], g, v)
+    assert H.rel_l2(g, g_ref) < 1e-6
+    assert H.rel_l2(v, v_ref) < 1e-6
+    v2 = np.zeros(d["vis"].shape, dtype=np.complex64)
+    idg.idg_grid_degrid_host(c["plan"], d["uvw"], d["vis"], d["aterms"], d["taper"], None, v2)
+    assert H.rel_l2(v2, v_ref) < 1e-6
+    # in place: the predicted visibilities may replace the measured ones
+    v3 = d["vis"].copy()
+    idg.idg_grid_degrid_host(c["plan"], d["uvw"], v3, d["aterms"], d["taper"], None, v3)
+    assert H.rel_l2(v3, v_ref) < 1e-6
+
+
 # ---------------------------------------------------------------------------------------------
 # full-size configurations in the launch configuration bench.py times: sampled subgrids / samples
 # ---------------------------------------------------------------------------------------------
