@@ -49,6 +49,11 @@ typedef enum {
                                    t / aterm_interval and c_pk varies inside the visibility loop (section 3.4,
                                    PAPER.md:247; Alg. 1); meta.aterm_slot = slot of the first timestep */
 
+#define IDG_PLAN_FP32_GRIDDER 4 /* flags: row a1 always runs the FP32 kernel.  Without it, plans with N = 32, per-block
+                                   A-terms, 8..128 channels per block and >= 256 visibilities per block on average run
+                                   Eq. 25 on the tensor cores with 22-bit (fp16 hi + lo) operands and FP32 accumulation:
+                                   ~8e-6 relative L2 against float64 instead of ~1e-6 (idg_plan_uses_tensor_cores) */
+
 /* Partitioning parameters (section 3.2; readings R10-R12).  All explicit. */
 typedef struct {
   int32_t grid_size;      /* L, even, >= subgrid_size */
@@ -57,7 +62,7 @@ typedef struct {
   int32_t max_timesteps;  /* per subgrid, >= 1 */
   int32_t max_channels;   /* per subgrid, power of two */
   int32_t aterm_interval; /* timesteps per A-term slot, >= 1 (R5: a block never spans two slots) */
-  int32_t flags;          /* IDG_PLAN_FORCE_BLOCKS | IDG_PLAN_SPAN_ATERMS or 0 */
+  int32_t flags;          /* IDG_PLAN_FORCE_BLOCKS | IDG_PLAN_SPAN_ATERMS | IDG_PLAN_FP32_GRIDDER or 0 */
   int32_t reserved;       /* must be 0 */
   double image_size;      /* S: direction-cosine extent of the image; grid cell = 1/S wavelengths */
   double w_step;          /* w-layer thickness in wavelengths; 0 -> w0 = 0 for every subgrid (R4) */

@@ -25,7 +25,7 @@ static int check_params(const idg_plan_params *p) {
   if (p->kernel_size <= 0 || p->kernel_size >= p->subgrid_size) return IDG_ERR_INVALID_ARG;
   if (p->max_timesteps < 1 || p->aterm_interval < 1) return IDG_ERR_INVALID_ARG;
   if (!is_pow2(p->max_channels) || p->max_channels > 256) return IDG_ERR_INVALID_ARG;
-  if (p->reserved != 0 || (p->flags & ~(IDG_PLAN_FORCE_BLOCKS | IDG_PLAN_SPAN_ATERMS))) return IDG_ERR_INVALID_ARG;
+  if (p->reserved != 0 || (p->flags & ~(IDG_PLAN_FORCE_BLOCKS | IDG_PLAN_SPAN_ATERMS | IDG_PLAN_FP32_GRIDDER))) return IDG_ERR_INVALID_ARG;
   if (!(p->image_size > 0.0) || !(p->image_size < 1.4) || !(p->w_step >= 0.0)) return IDG_ERR_INVALID_ARG;
   return IDG_OK;
 }

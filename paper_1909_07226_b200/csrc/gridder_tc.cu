@@ -415,7 +415,7 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
 bool gridder_tc_eligible(const idg_plan *plan) {
   // blocks shorter than ~256 visibilities do not amortise the pipeline fill and drain of a CTA (sweep: 128-visibility
   // blocks 0.64 here against 0.71 for the FFMA2 kernel; 256: 0.74 / 0.73; 512: 0.77 / 0.75; 2048: 0.83 / 0.75)
-  return plan->prm.subgrid_size == 32 && !(plan->prm.flags & IDG_PLAN_SPAN_ATERMS) && plan->min_n_chan >= 8 &&
+  return plan->prm.subgrid_size == 32 && !(plan->prm.flags & (IDG_PLAN_SPAN_ATERMS | IDG_PLAN_FP32_GRIDDER)) && plan->min_n_chan >= 8 &&
          plan->max_n_chan <= tc::VS &&                  // a staging batch holds at least one timestep of the block
          plan->P > 0 && plan->n_planned / plan->P >= 256;
 }

@@ -35,6 +35,7 @@ EARTH_ROTATION_RAD_S = 7.2921150e-5
 
 FLAG_FORCE_BLOCKS = 1
 FLAG_SPAN_ATERMS = 2
+FLAG_FP32_GRIDDER = 4
 
 
 @dataclasses.dataclass

@@ -724,3 +724,46 @@ def test_tensor_core_gridder_ragged_blocks(uneven, spread):
     err = np.array([H.rel_l2(got[p], ref[p]) for p in range(len(meta))])
     print("tensor-core gridder worst / median rel-L2: %.2e / %.2e" % (err.max(), np.median(err)))
     assert err.max() < TOL, (int(err.argmax()), float(err.max()))
+
+
+def test_fp32_gridder_flag_and_wide_blocks_leave_the_tensor_cores():
+    """IDG_PLAN_FP32_GRIDDER keeps row a1 on the FP32 kernel (closer to float64 than the 22-bit tensor-core operands);
+    a block with more channels than a staging batch of the tensor-core kernel holds (128) also takes the FP32 kernel.
+    Both against the oracle, and the flag's result against the tensor-core one."""
+    w = synth.make_workload("lofar", n_baselines=16, baseline_offset=300, n_time=64)
+    d = _np(w)
+    meta, _, _ = orc.plan(w.params, d["uvw"], d["freqs"], w.baselines)
+    plan_tc = idg.idg_plan_from_metadata(w.params, meta, w.freqs, w.B, w.T, w.n_stations)
+    prm32 = dataclasses.replace(w.params, flags=w.params.flags | synth.FLAG_FP32_GRIDDER)
+    plan32 = idg.idg_plan_from_metadata(prm32, meta, w.freqs, w.B, w.T, w.n_stations)
+    assert plan_tc.uses_tensor_cores() and not plan32.uses_tensor_cores()
+    wc = _cuda(w)
+    ref = orc.gridder(w.params, meta, d["uvw"], d["freqs"], d["vis"], d["aterms"], d["taper"])
+    out = {}
+    for name, plan in (("tc", plan_tc), ("fp32", plan32)):
+        sub = torch.zeros(ref.shape, dtype=torch.complex64, device="cuda")
+        idg.idg_gridder(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, sub)
+        torch.cuda.synchronize()
+        out[name] = sub.cpu().numpy()
+        assert H.rel_l2(out[name], ref) < TOL
+    assert H.rel_l2(out["tc"], out["fp32"]) < TOL
+    # 160 channels in one block: N = 32, per-block A-terms, long blocks -- and still not eligible
+    base = synth.make_workload("lofar", n_baselines=4, baseline_offset=300, n_time=32)
+    rng = np.random.default_rng(11)
+    f = base.freqs
+    freqs = np.linspace(f[0], f[-1], 160)                       # the same band in ten times as many channels
+    vis = (rng.standard_normal((base.B, base.T, 160, 4)) + 1j * rng.standard_normal((base.B, base.T, 160, 4))).astype(np.complex64)
+    wide = dataclasses.replace(base, freqs=freqs, vis=torch.from_numpy(vis))
+    dw = _np(wide)
+    mw, _, _ = orc.plan(wide.params, dw["uvw"], dw["freqs"], wide.baselines)
+    mw = mw.copy()
+    mw["chan_begin"] = 0
+    mw["n_chan"] = 160
+    plan_w = idg.idg_plan_from_metadata(wide.params, mw, wide.freqs, wide.B, wide.T, wide.n_stations)
+    assert not plan_w.uses_tensor_cores()
+    wcw = _cuda(wide)
+    refw = orc.gridder(wide.params, mw, dw["uvw"], dw["freqs"], dw["vis"], dw["aterms"], dw["taper"])
+    subw = torch.zeros(refw.shape, dtype=torch.complex64, device="cuda")
+    idg.idg_gridder(plan_w, wcw.uvw, wcw.vis, wcw.aterms, wcw.taper, subw)
+    torch.cuda.synchronize()
+    assert H.rel_l2(subw.cpu().numpy(), refw) < TOL
