@@ -50,7 +50,7 @@ typedef enum {
                                    PAPER.md:247; Alg. 1); meta.aterm_slot = slot of the first timestep */
 
 #define IDG_PLAN_FP32_GRIDDER 4 /* flags: row a1 always runs the FP32 kernel.  Without it, plans with N = 32, per-block
-                                   A-terms, 8..128 channels per block and >= 256 visibilities per block on average run
+                                   A-terms, 8..128 channels per block and >= 128 visibilities per block on average run
                                    Eq. 25 on the tensor cores with 22-bit (fp16 hi + lo) operands and FP32 accumulation:
                                    ~8e-6 relative L2 against float64 instead of ~1e-6 (idg_plan_uses_tensor_cores) */
 

@@ -410,14 +410,17 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
   if (warp == 8) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
 }
 
-// The tensor-core gridder serves per-block A-terms at N = 32 when every block has at least 8 channels (so that a
-// staging batch holds many more ring slots than the ring is deep); everything else takes gridder_kernel.
+// The tensor-core gridder serves per-block A-terms at N = 32 when every block has 8 to 128 channels (a ring slot is 8
+// channels of one timestep; a staging batch of 128 visibilities holds at least one timestep); everything else takes
+// gridder_kernel.
 bool gridder_tc_eligible(const idg_plan *plan) {
-  // blocks shorter than ~256 visibilities do not amortise the pipeline fill and drain of a CTA (sweep: 128-visibility
-  // blocks 0.64 here against 0.71 for the FFMA2 kernel; 256: 0.74 / 0.73; 512: 0.77 / 0.75; 2048: 0.83 / 0.75)
-  return plan->prm.subgrid_size == 32 && !(plan->prm.flags & (IDG_PLAN_SPAN_ATERMS | IDG_PLAN_FP32_GRIDDER)) && plan->min_n_chan >= 8 &&
+  // sweep (N = 32, 16 channels, fraction of the FP32 lane-op roofline, this kernel / the FFMA2 kernel) by block length:
+  // 128 visibilities 0.79 / 0.71; 256: 0.86 / 0.73; 512: 0.90 / 0.75; 2048: 0.93 / 0.75; 8192 at 64 channels: 0.97 / 0.76.
+  // Shorter blocks are not measured (the fixed cost per CTA -- allocation, block maximum, fill, drain, epilogue -- grows)
+  return plan->prm.subgrid_size == 32 && !(plan->prm.flags & (IDG_PLAN_SPAN_ATERMS | IDG_PLAN_FP32_GRIDDER)) &&
+         plan->min_n_chan >= 8 &&
          plan->max_n_chan <= tc::VS &&                  // a staging batch holds at least one timestep of the block
-         plan->P > 0 && plan->n_planned / plan->P >= 256;
+         plan->P > 0 && plan->n_planned / plan->P >= 128;
 }
 
 int launch_gridder_tc(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
