@@ -122,7 +122,7 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
   unsigned char *s_b = smem_dyn;                                          // [2][VS / 4][512]: B tiles, two staging buffers
   float4 *s_t = reinterpret_cast<float4 *>(smem_dyn + kSmemB);            // [2][VS / 4][2]: per timestep (u, v, w), (bu, bv, bw)
   float *s_kd = reinterpret_cast<float *>(smem_dyn + kSmemB + kSmemT);    // [VS]: kd per channel of the block, zero padded
-  __shared__ uint64_t bar_full[RING], bar_empty[RING], bar_done;
+  __shared__ uint64_t bar_empty[RING], bar_done;
   __shared__ uint32_t s_tmem, s_maxbits;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -138,7 +138,7 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (tid == 0) {
-    for (int s = 0; s < RING; ++s) { mbar_init(&bar_full[s], 8); mbar_init(&bar_empty[s], 1); }
+    for (int s = 0; s < RING; ++s) mbar_init(&bar_empty[s], 1);
     mbar_init(&bar_done, 1);
     s_maxbits = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -189,8 +189,8 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
       ql[k] = q.x; qm[k] = q.y; qn[k] = q.z;
     }
     uint32_t slot = 0, round = 0;                              // ring slot of the next step; times the ring went round
-    uint32_t empty_base = smem_u32(&bar_empty[0]), full_base = smem_u32(&bar_full[0]);
-    asm volatile("" : "+r"(empty_base), "+r"(full_base));      // kept in registers (not rematerialised per slot)
+    uint32_t empty_base = smem_u32(&bar_empty[0]);
+    asm volatile("" : "+r"(empty_base));                       // kept in a register (not rematerialised per slot)
     for (int t0 = 0, sb = 0; t0 < n_time; t0 += tb_max, ++sb) {
       const int tb = min(tb_max, n_time - t0), buf = sb & 1;
       unsigned char *bt = s_b + buf * (kSmemB / 2);
@@ -324,9 +324,10 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
           }
           asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
           tc_fence_before();
-          __syncwarp();
-          if (lane == 0)
-            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_base + 8u * slot) : "memory");
+          // hand-over on a named barrier: the generators only arrive, the issuing warp sleeps in bar.sync until all
+          // eight have (an mbarrier here cost the issuer ~170 instructions of polling per slot, 9 % of the kernel's)
+          static_assert(RING == 1, "one named barrier: a slot's phase ends before its next arrivals (empty barrier)");
+          asm volatile("bar.arrive 2, %0;" ::"n"(NT) : "memory");
           if (++slot == RING) { slot = 0; ++round; }
         }
       }
@@ -341,7 +342,7 @@ gridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__rest
       const uint32_t bt = smem_u32(s_b + (sb & 1) * (kSmemB / 2));
       for (int si = 0; si < tb * spt; ++si, ++gs) {
         const int slot = gs % RING;
-        mbar_wait_parked(&bar_full[slot], (gs / RING) & 1);
+        asm volatile("bar.sync 2, %0;" ::"n"(NT) : "memory");
         tc_fence_after();
         if (leader) {
           const uint32_t a0 = tmem + (uint32_t)(COLS_D + slot * COLS_SLOT);
