@@ -41,7 +41,8 @@ typedef enum {
   IDG_ERR_OUT_OF_MEMORY = -2,
   IDG_ERR_CUDA = -3,
   IDG_ERR_PLAN_MISMATCH = -4,
-  IDG_ERR_UNSUPPORTED_SUBGRID_SIZE = -5
+  IDG_ERR_UNSUPPORTED_SUBGRID_SIZE = -5,
+  IDG_ERR_SCRATCH_TOO_SMALL = -6 /* a *_static entry point was asked for more than its fixed scratch holds */
 } idg_status;
 
 #define IDG_PLAN_FORCE_BLOCKS 1 /* flags: blocks end only on max_timesteps / A-term slot (sweep mode) */
@@ -220,6 +221,20 @@ int idg_image_divide(void *image_dev, const float *cbar_dev, int32_t L, void *cu
  * axes, real part.  FP64 arithmetic, float32 result.  taper_dev [N][N] float32, cbar_dev [L][L] float32, N in
  * {16, 24, 32, 48}, L >= N even.  Asynchronous on cuda_stream; allocates (and frees, stream-ordered) 32 L N bytes. */
 int idg_image_taper(const float *taper_dev, int32_t N, float *cbar_dev, int32_t L, void *cuda_stream);
+/* The same result without any allocation, for callers that cannot call cudaMalloc (CUDA graph capture, serving
+ * loops): the 32 L N bytes of scratch live in a file-scope device array of the library, 8 MiB that every GPU which
+ * loads the library holds until exit.  Arguments, arithmetic and result as idg_image_taper (same kernels).
+ *   limit:   L * N <= IDG_IMAGE_TAPER_STATIC_MAX_LN (L <= 8192 at N = 32, L <= 5460 at N = 48); larger requests
+ *            return IDG_ERR_SCRATCH_TOO_SMALL before anything is launched -- use idg_image_taper for those
+ *   device:  the current device must be the one cuda_stream belongs to; the first call on each device resolves the
+ *            array's device address (cudaGetSymbolAddress: no allocation) -- make that call outside stream capture
+ *   sharing: every call on a device uses the SAME array, which keeps the previous call's contents (each call
+ *            overwrites what it reads, nothing needs clearing); two calls that overlap on the GPU -- different
+ *            streams, or captured into graphs that run concurrently -- race on it.  Calls on one stream are ordered.
+ * Calls no cudaMalloc / cudaFree / allocating library routine.  Errors: IDG_ERR_INVALID_ARG,
+ * IDG_ERR_SCRATCH_TOO_SMALL, IDG_ERR_CUDA. */
+#define IDG_IMAGE_TAPER_STATIC_MAX_LN 262144
+int idg_image_taper_static(const float *taper_dev, int32_t N, float *cbar_dev, int32_t L, void *cuda_stream);
 
 /* ---- optimal taper (offline input of the hot path) ----------------------------------
  * Section 4.3, Appendix A: the taper c[i][j] = a_i a_j (Eq. 30) whose effective

@@ -27,7 +27,7 @@ EXPORTS = (
     "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_grid_degrid_host", "idg_gridder", "idg_subgrid_fft",
     "idg_adder", "idg_splitter", "idg_splitter_ifft", "idg_degridder", "idg_image_w_accumulate", "idg_image_w_apply",
-    "idg_image_divide", "idg_image_taper", "idg_taper_optimal", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
+    "idg_image_divide", "idg_image_taper", "idg_image_taper_static", "idg_taper_optimal", "idg_grid_scalar", "idg_degrid_scalar", "idg_gridder_scalar", "idg_degridder_scalar")
 
 
 class IdgError(RuntimeError):
@@ -382,6 +382,19 @@ def idg_image_taper(taper, L: int, stream=None) -> torch.Tensor:
     _check(lib().idg_image_taper(_dev(taper, _F32, "taper"), ctypes.c_int32(N), _dev(out, _F32, "cbar"),
                                  ctypes.c_int32(int(L)), _stream(stream)), "idg_image_taper")
     return out
+
+
+IMAGE_TAPER_STATIC_MAX_LN = 262144      # IDG_IMAGE_TAPER_STATIC_MAX_LN of include/idg_b200.h
+
+
+def idg_image_taper_static(taper, cbar, stream=None) -> None:
+    """idg_image_taper without any allocation: writes c-bar into the caller's [L][L] float32 device tensor; the scratch
+    is a fixed 8 MiB device array of the library (L * N <= IMAGE_TAPER_STATIC_MAX_LN), shared by every call."""
+    N, L = int(taper.shape[0]), int(cbar.shape[0])
+    if tuple(taper.shape) != (N, N) or tuple(cbar.shape) != (L, L):
+        raise IdgError("taper must be [N][N] and cbar [L][L]")
+    _check(lib().idg_image_taper_static(_dev(taper, _F32, "taper"), ctypes.c_int32(N), _dev(cbar, _F32, "cbar"),
+                                        ctypes.c_int32(L), _stream(stream)), "idg_image_taper_static")
 
 
 def idg_taper_optimal(N: int, beta: float, device="cuda", stream=None):

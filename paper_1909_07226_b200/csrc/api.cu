@@ -161,6 +161,7 @@ const char *idg_strerror(int code) {
     case IDG_ERR_CUDA: return "CUDA error (see idg_last_cuda_error)";
     case IDG_ERR_PLAN_MISMATCH: return "metadata does not match the plan parameters or array shapes";
     case IDG_ERR_UNSUPPORTED_SUBGRID_SIZE: return "subgrid size must be 16, 24, 32 or 48";
+    case IDG_ERR_SCRATCH_TOO_SMALL: return "request exceeds the fixed scratch of the no-allocation (*_static) entry point";
     default: return "unknown error code";
   }
 }

@@ -11,6 +11,8 @@
 //                            l_x = (x - L/2) S / L  (Eq. 5), n' = sqrt(1 - l^2 - m^2) - 1 (R2)
 //   idg_image_w_apply:       out = in * exp(sign 2 pi i w0 n')            (prediction direction)
 //   idg_image_divide:        image[pol][y][x] /= cbar[y][x]               (c-bar: image-domain taper)
+#include <mutex>
+
 #include "common.cuh"
 
 namespace idg {
@@ -112,6 +114,37 @@ taper_image_kernel(float *__restrict__ cbar, const double2 *__restrict__ tmp, co
 
 using namespace idg;
 
+// ---- idg_image_taper_static: the same three kernels with their scratch in a file-scope device array, for callers
+// that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  The array
+// costs every GPU that loads the library 8 MiB until exit.  In HOST code `g_taper_scratch` is only a stand-in for
+// the device symbol, not a device address: its address is resolved once per device with cudaGetSymbolAddress (that
+// device current) and that pointer is what the kernels receive.
+namespace {
+
+constexpr int kStaticMaxLN = IDG_IMAGE_TAPER_STATIC_MAX_LN;             // L * N of the largest request served
+static __device__ __align__(256) double2 g_taper_scratch[2 * kStaticMaxLN];   // D [L][N], then tmp [L][N]
+
+constexpr int kMaxDevices = 64;
+std::mutex g_taper_scratch_mu;
+double2 *g_taper_scratch_ptr[kMaxDevices] = {};
+
+int taper_scratch_address(double2 **out) {
+  int dev = -1;
+  IDG_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return IDG_ERR_INVALID_ARG;
+  std::lock_guard<std::mutex> lock(g_taper_scratch_mu);
+  if (!g_taper_scratch_ptr[dev]) {
+    double2 *p = nullptr;
+    IDG_CUDA_TRY(cudaGetSymbolAddress((void **)&p, g_taper_scratch));
+    if (!p) return IDG_ERR_CUDA;
+    g_taper_scratch_ptr[dev] = p;
+  }
+  *out = g_taper_scratch_ptr[dev];
+  return IDG_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int idg_image_w_accumulate(void *acc_dev, const void *layer_dev, int32_t L, double image_size, double w0,
@@ -159,6 +192,27 @@ int idg_image_taper(const float *taper_dev, int32_t N, float *cbar_dev, int32_t 
   const cudaError_t e = cudaGetLastError();
   cudaFreeAsync(D, s);
   IDG_CUDA_TRY(e);
+  return IDG_OK;
+}
+
+int idg_image_taper_static(const float *taper_dev, int32_t N, float *cbar_dev, int32_t L, void *stream) {
+  if (!taper_dev || !cbar_dev || !(N == 16 || N == 24 || N == 32 || N == 48) || L < N || (L & 1))
+    return IDG_ERR_INVALID_ARG;
+  if ((int64_t)L * N > (int64_t)kStaticMaxLN) return IDG_ERR_SCRATCH_TOO_SMALL;
+  double2 *D = nullptr;
+  const int rc = taper_scratch_address(&D);
+  if (rc != IDG_OK) return rc;
+  double2 *tmp = D + (size_t)L * N;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int nb = (L * N + 127) / 128;
+  // every element of D and tmp that is read below is written first, in this call: nothing has to start at zero
+  taper_dirichlet_kernel<<<nb, 128, 0, s>>>(D, N, L);
+  count_launch();
+  taper_rows_kernel<<<nb, 128, 0, s>>>(tmp, D, taper_dev, N, L);
+  count_launch();
+  taper_image_kernel<<<dim3((L + 63) / 64, (L + 3) / 4), 256, 0, s>>>(cbar_dev, tmp, D, N, L);
+  count_launch();
+  IDG_CUDA_TRY(cudaGetLastError());
   return IDG_OK;
 }
 
