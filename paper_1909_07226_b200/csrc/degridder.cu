@@ -337,6 +337,7 @@ int launch_degridder(const idg_plan *plan, const float *uvw, const float2 *subgr
                      cudaStream_t stream, int64_t p0, int64_t np) {
   if (np < 0) np = plan->P - p0;
   if (np <= 0) return IDG_OK;
+  if (degridder_tc_eligible(plan)) return launch_degridder_tc(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
   switch (plan->prm.subgrid_size) {
     case 16: return launch_n<16>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
     case 24: return launch_n<24>(plan, uvw, subgrids, aterms, taper, vis_out, stream, p0, np);
