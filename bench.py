@@ -309,7 +309,8 @@ def measure_device_steps(idg, sharding, w, plan, steps, warmup, world, dev, samp
             "clocks": clocks}
 
 
-def kernel_rooflines(workload, stage_ms, alone_ms, planned, P, N, touched_px, hbm, hbm_source, tensor=False):
+def kernel_rooflines(workload, stage_ms, alone_ms, planned, P, N, touched_px, hbm, hbm_source, tensor=False,
+                     tensor_dg=False):
     """Per-kernel roofline objects: achieved = ALGORITHMIC work per launch / mean launch time inside the timed
     region (36 N^2 flop-equivalents per visibility for gridder / degridder; 64 N^2 bytes per
     subgrid for the FFT; 32 N^2 bytes per subgrid + 64 (32) bytes per touched grid pixel for adder (splitter))."""
@@ -333,7 +334,8 @@ def kernel_rooflines(workload, stage_ms, alone_ms, planned, P, N, touched_px, hb
 
     alu("gridder_tc_kernel (tcgen05 contraction; fraction of the FP32 lane-op roofline of the direct evaluation)" if tensor
         else "gridder_kernel", "gridder")
-    alu("degridder_kernel", "degridder")
+    alu("degridder_tc_kernel (tcgen05 contraction; fraction of the FP32 lane-op roofline of the direct evaluation)"
+        if tensor_dg else "degridder_kernel", "degridder")
     mem("subgrid_fft_kernel<N,fwd>", "subgrid_fft", 2 * sub_bytes, stage_ms["subgrid_fft"])
     mem("adder_kernel", "adder", sub_bytes + 2 * px, stage_ms["adder"])
     mem("subgrid_fft_kernel<N,inv,gather> (splitter + IFFT fused)", "splitter_ifft", sub_bytes + px,
@@ -470,7 +472,8 @@ def run_b200(args):
     meta = plan.metadata()
     touched_px = touched_grid_pixels(meta, N, L)
     tensor = plan.uses_tensor_cores()
-    kernels, alone = kernel_rooflines(args.workload, stage_ms, m["alone_ms"], planned, P, N, touched_px, hbm, hbm_source, tensor)
+    kernels, alone = kernel_rooflines(args.workload, stage_ms, m["alone_ms"], planned, P, N, touched_px, hbm, hbm_source, tensor,
+                                     plan.degridder_uses_tensor_cores())
     g = kernels[0]
     roofline = {"bound": "alu", "kernel": "gridder_tc_kernel" if tensor else "gridder_kernel", "achieved": g["achieved"], "peak": ALU_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": g["frac"], "traffic": g["traffic"], "peak_source": ALU_PEAK_SOURCE,
@@ -490,6 +493,7 @@ def run_b200(args):
     extra = {
         "correlations_per_s": 4.0 * value * 1e6,      # 4 polarisations per visibility (BASELINE.json's "0.5 G" reading)
         "gridder_on_tensor_cores": plan.uses_tensor_cores(),
+        "degridder_on_tensor_cores": plan.degridder_uses_tensor_cores(),
         "plan_ms": plan_ms, "n_subgrids_rank0": P, "n_vis_rank0": planned, "n_vis_total": total_vis, "n_skipped_rank0": skipped,
         "stage_ms": stage_ms,
         "grid_mvis_s": planned / ((stage_ms["gridder"] + stage_ms["subgrid_fft"] + stage_ms["adder"]) * 1e-3) / 1e6,
@@ -513,7 +517,8 @@ def run_b200(args):
         m2 = measure_device_steps(idg, sharding, w2, p2, max(5, args.steps), args.warmup, 1, dev)
         N2, L2 = w2.params.subgrid_size, w2.params.grid_size
         k2, _ = kernel_rooflines("lofar", m2["stage_ms"], m2["alone_ms"], planned2, P2, N2,
-                                 touched_grid_pixels(p2.metadata(), N2, L2), hbm, hbm_source, p2.uses_tensor_cores())
+                                 touched_grid_pixels(p2.metadata(), N2, L2), hbm, hbm_source, p2.uses_tensor_cores(),
+                                 p2.degridder_uses_tensor_cores())
         ms2 = m2["elapsed_ms"] / max(5, args.steps)
         extra["configs1_lofar"] = {"workload": WORKLOAD_NAMES["lofar"], "value": 2.0 * planned2 / (ms2 * 1e-3) / 1e6,
                                    "unit": UNIT, "ms_per_step": ms2, "stage_ms": m2["stage_ms"], "kernels": k2,

@@ -50,10 +50,12 @@ typedef enum {
                                    t / aterm_interval and c_pk varies inside the visibility loop (section 3.4,
                                    PAPER.md:247; Alg. 1); meta.aterm_slot = slot of the first timestep */
 
-#define IDG_PLAN_FP32_GRIDDER 4 /* flags: row a1 always runs the FP32 kernel.  Without it, plans with N = 32, per-block
-                                   A-terms, 8..128 channels per block and >= 128 visibilities per block on average run
-                                   Eq. 25 on the tensor cores with 22-bit (fp16 hi + lo) operands and FP32 accumulation:
-                                   ~8e-6 relative L2 against float64 instead of ~1e-6 (idg_plan_uses_tensor_cores) */
+#define IDG_PLAN_FP32_GRIDDER 4 /* flags: rows a1 and a6 always run the FP32 kernels.  Without it, plans with N = 32 and
+                                   per-block A-terms run Eq. 25 (8..128 channels per block, >= 128 visibilities per block
+                                   on average) and Alg. 2's inner loops (>= 384 visibilities per block on average) on the
+                                   tensor cores with 22-bit (fp16 hi + lo) operands and FP32 accumulation: ~8e-6 relative
+                                   L2 against float64 instead of ~1e-6 (idg_plan_uses_tensor_cores: bit 0 gridder, bit 1
+                                   degridder) */
 
 /* Partitioning parameters (section 3.2; readings R10-R12).  All explicit. */
 typedef struct {
@@ -133,8 +135,10 @@ int idg_plan_subgrids(const idg_plan *plan, void **subgrids_dev);
 /* Number of A-term slots the plan indexes: max over subgrids of the last slot + 1 (with IDG_PLAN_SPAN_ATERMS the
  * slot of a block's last timestep decides); 0 for an empty plan. */
 int idg_plan_aterm_slots(const idg_plan *plan, int32_t *n_slots);
-/* 1 if idg_gridder / idg_grid run this plan's contraction on the tensor cores (csrc/gridder_tc.cu: N = 32, one c_p
- * per block, at least 8 channels in every block, mean block of 256 visibilities or more), 0 if on the FP32 path. */
+/* Which of the plan's two contractions run on the tensor cores, as a bit mask: bit 0 (value 1) idg_gridder / idg_grid
+ * (csrc/gridder_tc.cu: N = 32, one c_p per block, 8 to 128 channels in every block, mean block of 128 visibilities or
+ * more), bit 1 (value 2) idg_degridder / idg_degrid (csrc/degridder_tc.cu: N = 32, one c_p per block, mean block of 384
+ * visibilities or more); 0: both on the FP32 path (always with IDG_PLAN_FP32_GRIDDER). */
 int idg_plan_uses_tensor_cores(const idg_plan *plan, int32_t *flag);
 /* w offset of a w layer, w0 = (w_index + 0.5) w_step, or 0 when w_step = 0 (Alg. 1, R4). */
 int idg_plan_w_offset(const idg_plan *plan, int32_t w_index, double *w0);

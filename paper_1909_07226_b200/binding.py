@@ -139,7 +139,13 @@ class Plan:
         """True if the gridder runs this plan on the tcgen05 path (idg_plan_uses_tensor_cores)."""
         f = ctypes.c_int32()
         _check(lib().idg_plan_uses_tensor_cores(self.handle, ctypes.byref(f)), "idg_plan_uses_tensor_cores")
-        return bool(f.value)
+        return bool(f.value & 1)
+
+    def degridder_uses_tensor_cores(self) -> bool:
+        """True if the degridder runs this plan on the tcgen05 path (bit 1 of idg_plan_uses_tensor_cores)."""
+        f = ctypes.c_int32()
+        _check(lib().idg_plan_uses_tensor_cores(self.handle, ctypes.byref(f)), "idg_plan_uses_tensor_cores")
+        return bool(f.value & 2)
 
     def w_offset(self, w_index: int) -> float:
         """w0 of a w layer (idg_plan_w_offset; Alg. 1, R4)."""

@@ -291,7 +291,7 @@ int idg_plan_aterm_slots(const idg_plan *pl, int32_t *n_slots) {
 
 int idg_plan_uses_tensor_cores(const idg_plan *pl, int32_t *flag) {
   if (!pl || !flag) return IDG_ERR_INVALID_ARG;
-  *flag = gridder_tc_eligible(pl) ? 1 : 0;
+  *flag = (gridder_tc_eligible(pl) ? 1 : 0) | (degridder_tc_eligible(pl) ? 2 : 0);
   return IDG_OK;
 }
 

@@ -101,7 +101,7 @@ int launch_gridder(const idg_plan *plan, const float *uvw, const float2 *vis, co
 bool gridder_tc_eligible(const idg_plan *plan);
 int launch_gridder_tc(const idg_plan *plan, const float *uvw, const float2 *vis, const float2 *aterms,
                       const float *taper, float2 *subgrids, cudaStream_t stream, int64_t p0, int64_t np);
-// tensor-core degridder (degridder_tc.cu): N = 32, per-block A-terms, mean block >= 96 visibilities
+// tensor-core degridder (degridder_tc.cu): N = 32, per-block A-terms, mean block >= 384 visibilities
 bool degridder_tc_eligible(const idg_plan *plan);
 int launch_degridder_tc(const idg_plan *plan, const float *uvw, const float2 *subgrids, const float2 *aterms,
                         const float *taper, float2 *vis_out, cudaStream_t stream, int64_t p0, int64_t np);

@@ -325,11 +325,14 @@ degridder_tc_kernel(const idg_subgrid_meta *__restrict__ meta, const float *__re
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
 }
 
-// N = 32, one A-term slot per block; any channel count (threads own visibilities).  Short blocks leave most lanes of
-// a 128-visibility tile idle: they stay on the FP32 kernel.
+// N = 32, one A-term slot per block; any channel count (threads own visibilities).  Short blocks pay the fixed cost
+// per subgrid (staging the B tiles twice, pipeline fill, the reduction over pixel parts) and leave lanes of their
+// 128-visibility tiles idle.  Sweep (N = 32, fraction of the FP32 roofline, this kernel / the FFMA2 kernel) by block
+// length: 128 visibilities 0.55 / 0.64; 256: 0.68 / 0.69; 512: 0.81 / 0.71 (16 channels) and 0.81 / 0.69 (4 channels);
+// 2048: 0.82 / 0.73; 8192: 0.82 / 0.72.
 bool degridder_tc_eligible(const idg_plan *plan) {
   return plan->prm.subgrid_size == 32 && !(plan->prm.flags & (IDG_PLAN_SPAN_ATERMS | IDG_PLAN_FP32_GRIDDER)) &&
-         plan->P > 0 && plan->n_planned / plan->P >= 96;
+         plan->P > 0 && plan->n_planned / plan->P >= 384;
 }
 
 int launch_degridder_tc(const idg_plan *plan, const float *uvw, const float2 *subgrids, const float2 *aterms,

@@ -767,3 +767,79 @@ def test_fp32_gridder_flag_and_wide_blocks_leave_the_tensor_cores():
     idg.idg_gridder(plan_w, wcw.uvw, wcw.vis, wcw.aterms, wcw.taper, subw)
     torch.cuda.synchronize()
     assert H.rel_l2(subw.cpu().numpy(), refw) < TOL
+
+
+# ---------------------------------------------------------------------------------------------
+# tensor-core degridder (csrc/degridder_tc.cu): N = 32, mean block >= 384 visibilities
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("spread", [False, True])
+def test_tensor_core_degridder_ragged_blocks(spread):
+    """Blocks of 45 to 1920 visibilities through the tcgen05 degridder: one tile of 128 visibilities with its pixels
+    split over four thread groups, two tiles over two each, three and four tiles, and more than four (several rounds
+    that stage the B tiles again), channel counts 5 / 9 / 16 so that tiles do not end on timestep boundaries, ragged
+    last tiles.  Every visibility against the float64 oracle, per block; `spread` gives the subgrid images of a plan
+    twelve orders of magnitude of dynamic range (the kernel scales every subgrid by a power of two into the fp16
+    range and splits hi + lo), judged per block like the others."""
+    w = synth.make_workload("lofar", n_baselines=24, baseline_offset=300, n_time=128)
+    rng = np.random.default_rng(6)
+    d = _np(w)
+    meta, _, _ = orc.plan(w.params, d["uvw"], d["freqs"], w.baselines)
+    meta = meta.copy()
+    meta["n_chan"] = rng.choice([5, 9, 16, 16], len(meta))
+    meta["chan_begin"] = 0
+    meta["n_time"] = np.minimum(meta["n_time"], rng.choice([9, 15, 23, 40, 64, 120, 120], len(meta)))
+    plan = idg.idg_plan_from_metadata(w.params, meta, w.freqs, w.B, w.T, w.n_stations)
+    assert plan.degridder_uses_tensor_cores()
+    nv = meta["n_time"].astype(np.int64) * meta["n_chan"]
+    assert nv.min() <= 128 and ((nv > 128) & (nv <= 256)).any() and ((nv > 256) & (nv <= 512)).any() and nv.max() > 512
+    N = w.params.subgrid_size
+    P = len(meta)
+    img = (rng.standard_normal((P, 4, N, N)) + 1j * rng.standard_normal((P, 4, N, N))).astype(np.complex64)
+    if spread:
+        img *= (10.0 ** rng.uniform(-6, 6, P))[:, None, None, None].astype(np.float32)
+    ref = orc.degridder(w.params, meta, d["uvw"], d["freqs"], img.astype(np.complex128), d["aterms"], d["taper"], w.B)
+    wc = _cuda(w)
+    out = torch.zeros(wc.vis.shape, dtype=torch.complex64, device="cuda")
+    idg.idg_degridder(plan, wc.uvw, torch.from_numpy(img).cuda(), wc.aterms, wc.taper, out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    # blocks of one baseline overlap in (time, channel) after the edits above: the last writer wins in both
+    # implementations only if they run in the same order, so judge the blocks nobody overwrites
+    owner = -np.ones((w.B, w.T, len(w.freqs)), dtype=np.int64)
+    for p in range(P):
+        mm = meta[p]
+        owner[mm["baseline"], mm["time_begin"]:mm["time_begin"] + mm["n_time"], 0:mm["n_chan"]] = p
+    err = []
+    for p in range(P):
+        mm = meta[p]
+        sl = (mm["baseline"], slice(mm["time_begin"], mm["time_begin"] + mm["n_time"]), slice(0, mm["n_chan"]))
+        if (owner[sl] == p).all():
+            err.append(H.rel_l2(got[sl], ref[sl]))
+    err = np.array(err)
+    assert len(err) > P // 2
+    print("tensor-core degridder worst / median rel-L2 over %d blocks: %.2e / %.2e" % (len(err), err.max(), np.median(err)))
+    assert err.max() < TOL
+
+
+def test_fp32_flag_keeps_the_degridder_off_the_tensor_cores():
+    w = synth.make_workload("lofar", n_baselines=8, baseline_offset=300, n_time=128)
+    d = _np(w)
+    meta, _, _ = orc.plan(w.params, d["uvw"], d["freqs"], w.baselines)
+    plan_tc = idg.idg_plan_from_metadata(w.params, meta, w.freqs, w.B, w.T, w.n_stations)
+    prm32 = dataclasses.replace(w.params, flags=w.params.flags | synth.FLAG_FP32_GRIDDER)
+    plan32 = idg.idg_plan_from_metadata(prm32, meta, w.freqs, w.B, w.T, w.n_stations)
+    assert plan_tc.degridder_uses_tensor_cores() and not plan32.degridder_uses_tensor_cores()
+    rng = np.random.default_rng(8)
+    N, P = w.params.subgrid_size, len(meta)
+    img = (rng.standard_normal((P, 4, N, N)) + 1j * rng.standard_normal((P, 4, N, N))).astype(np.complex64)
+    ref = orc.degridder(w.params, meta, d["uvw"], d["freqs"], img.astype(np.complex128), d["aterms"], d["taper"], w.B)
+    wc = _cuda(w)
+    res = {}
+    for name, plan in (("tc", plan_tc), ("fp32", plan32)):
+        out = torch.zeros(wc.vis.shape, dtype=torch.complex64, device="cuda")
+        idg.idg_degridder(plan, wc.uvw, torch.from_numpy(img).cuda(), wc.aterms, wc.taper, out)
+        torch.cuda.synchronize()
+        res[name] = out.cpu().numpy()
+        assert H.rel_l2(res[name], ref) < TOL
+    assert H.rel_l2(res["tc"], res["fp32"]) < TOL
