@@ -46,9 +46,9 @@ HBM_FALLBACK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback w
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of the
 # same workload (profiles/r02_ncu_summary.md); None where no capture of that workload exists.
 NCU_TRAFFIC_BYTES = {
-    "ska": {"gridder": int((16.073193 + 8.691625) * 1e9), "degridder": int((16.922555 + 4.237091) * 1e9),
+    "ska": {"gridder": int((16.009295 + 8.690905) * 1e9), "degridder": int((16.891421 + 4.243539) * 1e9),
             "subgrid_fft": None,      # ncu returned no DRAM counters for this launch (two captures); time and bytes only
-            "adder": int((8.861694 + 0.119106) * 1e9), "splitter_ifft": int((0.340902 + 8.652198) * 1e9)},
+            "adder": int((8.861878 + 0.119561) * 1e9), "splitter_ifft": int((0.336635 + 8.652087) * 1e9)},
 }
 
 WORKLOAD_NAMES = {
