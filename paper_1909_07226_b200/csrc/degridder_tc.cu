@@ -12,15 +12,18 @@
 //
 // Orientation: the contraction index is the pixel, so here the THREADS own visibilities: a group of 128 threads
 // (4 warps = the 128 lanes of tensor memory) owns a tile of 128 visibilities of the block; a thread evaluates its
-// visibility's phase U l + V m + W n' (U = 2 pi (u k_c - u0) etc., FP64 once per tile) for 8 pixels of a row at a
-// time (l, m are affine in the pixel index: two FMAs per pixel, n' from a shared-memory table), takes sin/cos.approx,
-// splits, and writes its row of two A tiles (8 pixels = 2 x K16) with one tcgen05.st.  The B operand of the whole
-// subgrid -- 256 tiles of 512 bytes -- is staged once per subgrid (128 KB: one CTA of 8 groups = 1024 threads per SM).
-// One warp of the group (they take turns) waits for the other three on a named barrier, issues the slot's two MMAs
-// into the group's accumulator D[128 x 16] and commits them to the group's "empty" mbarrier, which the group tests
-// before its next store.  Blocks with fewer than 8 tiles split the pixels of a tile over several groups; the partial
-// sums meet in shared memory.  Unlike the gridder there is no rotation recurrence (neighbouring pixels do not differ
-// by a constant phase: n' is not affine), so the kernel is bound by the two MUFU operations per (visibility, pixel).
+// visibility's phase a (x - 16) + b (y - 16) + W n' (a = 2 pi (u k_c - u0) S/N etc., FP64 once per tile; two FMAs per
+// pixel, n' from a shared-memory table) for 16 pixels of a row at a time, takes sin/cos.approx, splits, and writes its
+// row of four A tiles (16 pixels = 4 x K16) with two tcgen05.st.x16.  The B operand -- 512 bytes per 4 pixels, 128 KB
+// for a subgrid -- is staged in shared memory for HALF a subgrid at a time (64 KB), so that two CTAs of four groups
+// (512 threads, 64 registers, 256 tensor-memory columns) share an SM: a round of four visibility tiles stages both
+// halves and keeps its accumulators D[128 x 16] in tensor memory across them; blocks of more than 512 visibilities
+// take several rounds.  One warp of the group (they take turns) waits for the other three on a named barrier, issues
+// the slot's four MMAs and commits them to the group's "empty" mbarrier, which the group tests before its next store.
+// Blocks with fewer than four tiles split the pixels of a tile over several groups; the partial sums meet in shared
+// memory.  Unlike the gridder there is no rotation recurrence (neighbouring pixels do not differ by a constant phase:
+// n' is not affine), so every phasor costs two MUFU operations: the kernel is bound by the XU pipe and by the 32 warps
+// per SM that 64 registers allow.  Measurements and variants: profiles/r02_experiments.md section 8.
 #include <cuda_fp16.h>
 
 #include "common.cuh"
