@@ -74,8 +74,8 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait_addr(uint32_t addr, uint32_t parity) {
   uint32_t ok = 0;
   for (int spins = 0; spins < (1 << 26); ++spins) {
-    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                 : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(addr), "r"(parity), "r"(500u) : "memory");      // parked up to 500 ns between polls
     if (ok) return;
   }
   __trap();
