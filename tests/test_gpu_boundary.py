@@ -262,12 +262,12 @@ def test_guard_bands_planner_made_plan_with_skips():
 
 
 def test_host_entry_points_with_the_tensor_core_gridder_in_chunks():
-    """A planner-made N = 32 plan that takes the tensor-core gridder, through the chunked host-buffer calls (24
+    """A planner-made N = 32 plan that takes the tensor-core gridder and degridder, through the chunked host-buffer calls (24
     baseline ranges, each a launch on a sub-range of the subgrids) against the one-launch device calls."""
     w = synth.make_workload("lofar", n_baselines=96, baseline_offset=200, n_time=128)
     wc = w.to("cuda")
     plan = idg.idg_plan_create(w.params, wc.uvw, w.freqs, w.baselines, w.n_stations)
-    assert plan.uses_tensor_cores()
+    assert plan.uses_tensor_cores() and plan.degridder_uses_tensor_cores()
     L = w.params.grid_size
     g_dev = torch.zeros((4, L, L), dtype=torch.complex64, device="cuda")
     idg.idg_grid(plan, wc.uvw, wc.vis, wc.aterms, wc.taper, g_dev)
