@@ -489,6 +489,14 @@ def run_b200(args):
             "uniform_register_operands_tflops": mix[1], "scalar_ffma_tflops": mix[2]}
     except Exception as exc:      # reporting only
         roofline["measured_mix_peak"] = {"error": str(exc)}
+    try:     # issue rate of the tensor-core kernels' MMA, measured live (csrc/mmabench.cu)
+        roofline["measured_mma_cycles"] = {
+            "n16_1cta": idg.idg_bench_mma_rate(16, 1), "n16_4cta": idg.idg_bench_mma_rate(16, 4),
+            "n64": idg.idg_bench_mma_rate(64, 1), "n128": idg.idg_bench_mma_rate(128, 1), "n256": idg.idg_bench_mma_rate(256, 1),
+            "what": "SM cycles per tcgen05.mma.cta_group::1.kind::f16 (M128 x N x K16, A in tensor memory) and SM; "
+                    "the kernels use N = 16: 512 (visibility, pixel) pairs per MMA"}
+    except Exception as exc:      # reporting only
+        roofline["measured_mma_cycles"] = {"error": str(exc)}
     grid_bytes = 8.0 * 4 * L * L
     extra = {
         "correlations_per_s": 4.0 * value * 1e6,      # 4 polarisations per visibility (BASELINE.json's "0.5 G" reading)

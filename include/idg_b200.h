@@ -106,6 +106,14 @@ long long idg_kernel_launches(void);
  * upper bound the real kernel cannot reach from CUDA C); 2: 16 scalar FMA instead of 8 packed ones.
  * Synchronises cuda_stream; allocates and frees a small buffer. */
 int idg_bench_instruction_mix(int32_t iters, int32_t variant, double *tflop_equiv_per_s, void *cuda_stream);
+/* Measurement aid for the tensor-core kernels (Eq. 25 PAPER.md:230-235 and Alg. 2 PAPER.md:333-345 as contractions):
+ * the issue rate of tcgen05.mma.cta_group::1.kind::f16 with M = 128, K = 16, N = n in {16, 64, 128, 256}, A operand in
+ * tensor memory, B operand in shared memory -- the form csrc/gridder_tc.cu and csrc/degridder_tc.cu use with N = 16.
+ * ctas_per_sm CTAs (1..4 for n <= 64, 1..2 for n = 128, 1 for n = 256) each issue n_mma MMAs (a multiple of 8) back
+ * to back; the result is SM cycles per MMA, per SM.  Synchronises cuda_stream; allocates and frees a small buffer.
+ * Errors: IDG_ERR_INVALID_ARG, IDG_ERR_CUDA. */
+int idg_bench_mma_rate(int32_t n, int32_t ctas_per_sm, int32_t n_mma, double *cycles_per_mma_per_sm,
+                       void *cuda_stream);
 
 /* ---- planner (a0): section 3.2, Fig. 2; readings R10-R12 -----
  * Partitions every baseline's (time x channel) samples into blocks whose uv extent in grid

@@ -22,7 +22,7 @@ META_DTYPE = np.dtype([(n, "<i4") for n in (
 assert META_DTYPE.itemsize == 48
 
 EXPORTS = (
-    "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_bench_instruction_mix", "idg_plan_create", "idg_plan_from_metadata",
+    "idg_strerror", "idg_last_cuda_error", "idg_kernel_launches", "idg_bench_instruction_mix", "idg_bench_mma_rate", "idg_plan_create", "idg_plan_from_metadata",
     "idg_plan_size", "idg_plan_metadata", "idg_plan_subgrids", "idg_plan_aterm_slots", "idg_plan_w_offset", "idg_plan_uses_tensor_cores",
     "idg_plan_destroy", "idg_grid",
     "idg_degrid", "idg_grid_host", "idg_degrid_host", "idg_grid_degrid_host", "idg_gridder", "idg_subgrid_fft",
@@ -196,6 +196,14 @@ def idg_bench_instruction_mix(iters: int = 4096, variant: int = 0, stream=None) 
     _check(lib().idg_bench_instruction_mix(ctypes.c_int32(int(iters)), ctypes.c_int32(int(variant)), ctypes.byref(out),
                                            _stream(stream)),
            "idg_bench_instruction_mix")
+    return float(out.value)
+
+
+def idg_bench_mma_rate(n: int = 16, ctas_per_sm: int = 1, n_mma: int = 8000, stream=None) -> float:
+    """SM cycles per tcgen05.mma (kind::f16, M128 x N x K16, A in tensor memory) and SM (csrc/mmabench.cu)."""
+    out = ctypes.c_double()
+    _check(lib().idg_bench_mma_rate(ctypes.c_int32(int(n)), ctypes.c_int32(int(ctas_per_sm)), ctypes.c_int32(int(n_mma)),
+                                    ctypes.byref(out), _stream(stream)), "idg_bench_mma_rate")
     return float(out.value)
 
 

@@ -16,7 +16,7 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 BUILD_DIR = os.path.join(_HERE, "build")
 LIB_PATH = os.path.join(_HERE, "libidg_b200.so")
 
-SOURCES = ("plan.cu", "gridder.cu", "gridder_tc.cu", "degridder.cu", "degridder_tc.cu", "subgrid_fft.cu", "adder.cu", "image.cu", "scalar.cu", "mixbench.cu", "taper.cu", "api.cu", "api_run.cu")
+SOURCES = ("plan.cu", "gridder.cu", "gridder_tc.cu", "degridder.cu", "degridder_tc.cu", "subgrid_fft.cu", "adder.cu", "image.cu", "scalar.cu", "mixbench.cu", "mmabench.cu", "taper.cu", "api.cu", "api_run.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-I", INCLUDE]
 

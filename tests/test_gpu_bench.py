@@ -62,3 +62,17 @@ def test_two_ranks_shard_one_workload_and_reduce_the_grid():
     assert c["bytes"] == 8 * 4 * 256 * 256 and c["ms"] > 0
     assert d["detail"]["stage_ms"]["allreduce_grid"] > 0
     assert "2 ranks" in d["config"]["parallelism"]
+
+
+def test_mma_rate_probe_reports_the_measured_floor():
+    """idg_bench_mma_rate (csrc/mmabench.cu): the M128 x N x K16 MMA with A in tensor memory runs at M N / 256 cycles
+    from N = 64 up and at ~9 cycles for N = 16, whatever the number of CTAs per SM (profiles/r02_experiments.md
+    section 7); loose bounds, the probe is a measurement aid."""
+    from paper_1909_07226_b200 import binding as idg
+    c16 = idg.idg_bench_mma_rate(16, 1)
+    c16x4 = idg.idg_bench_mma_rate(16, 4)
+    c256 = idg.idg_bench_mma_rate(256, 1)
+    assert 4.0 < c16 < 16.0 and 4.0 < c16x4 < 16.0
+    assert 100.0 < c256 < 160.0
+    with pytest.raises(idg.IdgError):
+        idg.idg_bench_mma_rate(32, 1)
