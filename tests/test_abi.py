@@ -62,3 +62,14 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "idg_oracle" not in src and "from oracle" not in src and "import oracle" not in src, f
+
+
+def test_binding_constants_match_the_header():
+    """Limits and flags that the Python binding repeats are the header's."""
+    from paper_1909_07226_b200 import binding, synth
+    text = open(os.path.join(ROOT, "include", "idg_b200.h")).read()
+    defs = dict(re.findall(r"#define\s+(IDG_[A-Z_0-9]+)\s+(\d+)", text))
+    assert int(defs["IDG_IMAGE_TAPER_STATIC_MAX_LN"]) == binding.IMAGE_TAPER_STATIC_MAX_LN
+    assert int(defs["IDG_PLAN_FORCE_BLOCKS"]) == synth.FLAG_FORCE_BLOCKS
+    assert int(defs["IDG_PLAN_SPAN_ATERMS"]) == synth.FLAG_SPAN_ATERMS
+    assert int(defs["IDG_PLAN_FP32_GRIDDER"]) == synth.FLAG_FP32_GRIDDER
